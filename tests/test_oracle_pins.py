@@ -1,0 +1,343 @@
+"""Pins for the CPU oracle (no GPU): each test checks oracle/ against something OTHER than itself --
+values printed in SURVEY.md 8(c) worked examples (tests/golden/), closed forms, brute-force vertex
+enumeration, HiGHS, dense numpy algebra, and textbook invariants of PDHG.  DESIGN.md lists which
+reading (R1..R14) each pin covers and which remain 'parity unpinned' (R10, R11 decisions)."""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from workloads import tiny, uc_config, fix_commitment
+from workloads.lp import from_dense
+
+from helpers import read_golden_rows, vertex_enumeration, highs, dense_kkt, rel_l2
+
+
+def _f(s):
+    return float(s)
+
+
+# ------------------------------------------------------------------ R2..R6: the PDHG step
+def test_worked_1x1_step_example_matches_golden():
+    rows = read_golden_rows("pdhg_step_1x1.txt")
+    lp = tiny.one_by_one()
+    s = oracle.solve(lp, fixed_iterations=len(rows), ruiz_iters=0, pc_alpha=0.0,
+                     trace_attempts=len(rows), dump=len(rows))
+    x_cur, y_cur = 0.0, 0.0
+    eta = 1.0
+    for r, a, xd, yd in zip(rows, s.attempts, s.dump_x[:, 0], s.dump_y[:, 0]):
+        k, x_new, y_new, eta_bar, acc, eta_next = int(r[0]), _f(r[1]), _f(r[2]), _f(r[3]), int(r[4]), _f(r[5])
+        assert a["eta_used"] == pytest.approx(eta, rel=2e-9)
+        assert a["accepted"] == acc, f"attempt {k}"
+        if not math.isnan(eta_bar):
+            assert a["eta_bar"] == pytest.approx(eta_bar, rel=2e-9)
+        assert a["eta_next"] == pytest.approx(eta_next, rel=2e-9)
+        if acc:
+            x_cur, y_cur = x_new, y_new
+        assert xd == pytest.approx(x_cur, rel=2e-9, abs=1e-12)      # iterate after attempt k
+        assert yd == pytest.approx(y_cur, rel=2e-9, abs=1e-12)
+        eta = eta_next
+    # limit point of the same example: x*=1, y*=1, objective 1
+    s = oracle.solve(lp, eps_rel=1e-10, eps_abs=1e-10, ruiz_iters=0, pc_alpha=0.0)
+    assert s.status == 0 and s.x[0] == pytest.approx(1.0, abs=1e-8) and s.y[0] == pytest.approx(1.0, abs=1e-8)
+
+
+def test_step_first_attempts_by_hand():
+    """k=1..3 of the 1x1 example re-derived here from the update formulas with plain floats."""
+    lp = tiny.one_by_one()
+    s = oracle.solve(lp, fixed_iterations=3, ruiz_iters=0, pc_alpha=0.0, trace_attempts=3)
+    e1 = 1.0 + 2.0 ** -0.6                      # k=1: x'=0, y'=1, eta_bar=inf -> grow
+    e2 = (1.0 + 3.0 ** -0.6) * e1               # k=2: x'=0, y'=1+e1
+    y2 = 1.0 + e1
+    x3 = e2 * (y2 - 1.0)                        # k=3: x' = 0 - e2 (1 - y2)
+    dy = -y2                                    # y' = max(y2 + e2 (1 - 2 x3), 0) = 0
+    ebar3 = (x3 * x3 + dy * dy) / (2.0 * abs(dy * x3))
+    e3 = (1.0 - 4.0 ** -0.3) * ebar3
+    assert y2 + e2 * (1 - 2 * x3) < 0
+    assert s.attempts["eta_next"][0] == pytest.approx(e1, rel=1e-14)
+    assert s.attempts["eta_next"][1] == pytest.approx(e2, rel=1e-14)
+    assert s.attempts["eta_bar"][2] == pytest.approx(ebar3, rel=1e-14)
+    assert s.attempts["accepted"].tolist() == [1, 1, 0]
+    assert s.attempts["eta_next"][2] == pytest.approx(e3, rel=1e-14)
+
+
+# ------------------------------------------------------------------ R1: preconditioning
+def test_worked_2x2_preconditioner_matches_golden():
+    g = {r[0]: np.array([float(v) for v in r[1:]]) for r in read_golden_rows("precond_2x2.txt")}
+    lp = tiny.precond_2x2()
+    vs, Dr, Dc = oracle.precondition(lp, ruiz_iters=10, pc_alpha=0.0)
+    np.testing.assert_allclose(Dr, g["ruiz_Dr"], rtol=2e-10)
+    np.testing.assert_allclose(Dc, g["ruiz_Dc"], rtol=2e-10)
+    np.testing.assert_allclose(vs, g["ruiz_K"], rtol=2e-10)
+    vs2, _, _ = oracle.precondition(lp, ruiz_iters=2, pc_alpha=0.0)     # passes 3..10 change nothing
+    np.testing.assert_allclose(vs2, vs, rtol=1e-15)
+    vs, Dr, Dc = oracle.precondition(lp, ruiz_iters=10, pc_alpha=1.0)
+    np.testing.assert_allclose(Dr, g["final_Dr"], rtol=2e-10)
+    np.testing.assert_allclose(Dc, g["final_Dc"], rtol=2e-10)
+    np.testing.assert_allclose(vs, g["final_K"], rtol=2e-10)
+    Kt = np.array([[vs[0], vs[1]], [0.0, vs[2]]])
+    assert np.linalg.svd(Kt, compute_uv=False)[0] == pytest.approx(1.0, abs=1e-12)
+
+
+def test_ruiz_on_diagonal_matrix_closed_form():
+    a = np.array([4.0, -9.0, 0.25, 1e-4, -1e4])
+    lp = from_dense(np.diag(a), ["E"] * 5, np.ones(5), np.ones(5), -np.ones(5), np.ones(5))
+    for iters in (1, 10):
+        vs, Dr, Dc = oracle.precondition(lp, ruiz_iters=iters, pc_alpha=0.0)
+        np.testing.assert_allclose(Dr, np.sqrt(np.abs(a)), rtol=1e-15)
+        np.testing.assert_allclose(Dc, np.sqrt(np.abs(a)), rtol=1e-15)
+        np.testing.assert_allclose(vs, np.sign(a), rtol=1e-15)
+
+
+@pytest.mark.parametrize("seed", [0, 1, 2])
+def test_preconditioner_identities_and_operator_norm(seed):
+    lp = tiny.small_random(8, 6, seed, density=0.6)
+    vs, Dr, Dc = oracle.precondition(lp)
+    K = lp.dense()
+    Kt = np.zeros_like(K)
+    rows = np.repeat(np.arange(lp.m), np.diff(lp.row_ptr))
+    Kt[rows, lp.col_idx] = vs
+    np.testing.assert_allclose(Kt * Dr[:, None] * Dc[None, :], K, rtol=4e-15, atol=0)     # K = Dr Kt Dc
+    assert np.linalg.svd(Kt, compute_uv=False)[0] <= 1.0 + 1e-12                          # Pock-Chambolle lemma
+    # Ruiz alone equilibrates: row and column inf-norms approach 1, monotonically
+    dev_prev = np.inf
+    for it in (1, 3, 10):
+        vr, _, _ = oracle.precondition(lp, ruiz_iters=it, pc_alpha=0.0)
+        Kr = np.zeros_like(K); Kr[rows, lp.col_idx] = vr
+        dev = max(np.abs(np.abs(Kr).max(axis=1) - 1).max(), np.abs(np.abs(Kr).max(axis=0) - 1).max())
+        assert dev <= dev_prev + 1e-15
+        dev_prev = dev
+    assert dev_prev < 0.05
+
+
+def test_preconditioner_on_uc_config0_operator_norm_and_empty_handling():
+    import scipy.sparse as sp
+    import scipy.sparse.linalg as spl
+    lp = uc_config(0)
+    vs, Dr, Dc = oracle.precondition(lp)
+    Kt = sp.csr_matrix((vs, lp.col_idx, lp.row_ptr), shape=(lp.m, lp.n))
+    smax = spl.svds(Kt, k=1, return_singular_vectors=False)[0]
+    assert smax <= 1.0 + 1e-10
+    assert np.all(Dr > 0) and np.all(Dc > 0) and np.all(np.isfinite(Dr)) and np.all(np.isfinite(Dc))
+    # an LP with an empty row and an empty column: scaling factor 1 there
+    lp2 = from_dense([[2.0, 0.0, 0.0], [0.0, 0.0, 0.0]], ["G", "G"], [0.0, -1.0], [1.0, 1.0, 1.0],
+                     [0.0] * 3, [1.0] * 3)
+    _, Dr2, Dc2 = oracle.precondition(lp2)
+    assert Dr2[1] == 1.0 and Dc2[1] == 1.0 and Dc2[2] == 1.0
+
+
+# ------------------------------------------------------------------ SpMV pair
+def test_spmv_pair_dense_and_adjoint():
+    rng = np.random.default_rng(5)
+    lp = tiny.small_random(8, 6, 3)
+    K = lp.dense()
+    x = rng.standard_normal(lp.n); y = rng.standard_normal(lp.m)
+    np.testing.assert_allclose(oracle.spmv(lp, x), K @ x, rtol=1e-14, atol=1e-15)
+    np.testing.assert_allclose(oracle.spmv_t(lp, y), K.T @ y, rtol=1e-14, atol=1e-15)
+    lp = uc_config(0)
+    x = rng.standard_normal(lp.n); y = rng.standard_normal(lp.m)
+    lhs, rhs = y @ oracle.spmv(lp, x), oracle.spmv_t(lp, y) @ x
+    assert abs(lhs - rhs) <= 1e-13 * max(abs(lhs), 1.0) * 10
+    np.testing.assert_allclose(oracle.spmv(lp, x), lp.to_scipy() @ x, rtol=1e-13, atol=1e-13)
+    np.testing.assert_allclose(oracle.spmv_t(lp, y), lp.to_scipy().T @ y, rtol=1e-13, atol=1e-13)
+
+
+# ------------------------------------------------------------------ closed forms
+@pytest.mark.parametrize("rows", [0, 3])
+def test_box_only_lp_closed_form(rows):
+    lp = tiny.box_only(7, seed=1, with_rows=rows)
+    s = oracle.solve(lp, eps_rel=1e-9, eps_abs=1e-9)
+    expect = np.where(lp.c > 0, lp.l, np.where(lp.c < 0, lp.u, np.clip(0.0, lp.l, lp.u)))
+    assert s.status == 0
+    np.testing.assert_allclose(s.x, expect, atol=1e-9)
+    assert s.primal_obj == pytest.approx(np.minimum(lp.c * lp.l, lp.c * lp.u).sum(), rel=1e-9)
+    assert s.iterations <= 64 * 4                      # reached in finitely many attempts
+
+
+@pytest.mark.parametrize("seed", [0, 1, 2, 3])
+def test_single_bus_economic_dispatch_is_merit_order(seed):
+    lp, pmax, cost, d = tiny.economic_dispatch(6, seed)
+    order = np.argsort(cost)
+    p = np.zeros(6); left = d; marginal = None
+    for g in order:
+        p[g] = min(pmax[g], left); left -= p[g]
+        if marginal is None and left <= 1e-15:
+            marginal = cost[g]
+    s = oracle.solve(lp, eps_rel=1e-9, eps_abs=1e-9)
+    assert s.status == 0
+    np.testing.assert_allclose(s.x, p, atol=2e-6)
+    assert s.primal_obj == pytest.approx(float(cost @ p), rel=1e-7)
+    assert s.y[0] == pytest.approx(marginal, rel=1e-5)             # balance dual = marginal unit's cost
+
+
+def test_worked_two_variable_lp():
+    s = oracle.solve(tiny.two_var(), eps_rel=1e-10, eps_abs=1e-10)
+    assert s.status == 0
+    np.testing.assert_allclose(s.x, [1.0, 3.0], atol=1e-7)
+    np.testing.assert_allclose(s.y, [1.0], atol=1e-7)
+    assert s.primal_obj == pytest.approx(-7.0, abs=1e-7) and s.dual_obj == pytest.approx(-7.0, abs=1e-7)
+
+
+def test_free_and_one_sided_variables():
+    s = oracle.solve(tiny.free_var_lp(), eps_rel=1e-10, eps_abs=1e-10)
+    assert s.status == 0
+    np.testing.assert_allclose(s.x, [1.0, 0.0, 1.0], atol=1e-6)
+    np.testing.assert_allclose(s.y, [1.0, 1.0], atol=1e-6)
+    assert s.dual_obj == pytest.approx(1.0, abs=1e-6)
+
+
+# ------------------------------------------------------------------ brute force on tiny LPs
+@pytest.mark.parametrize("n,m,seed", [(4, 3, 0), (5, 4, 1), (6, 4, 2), (6, 5, 3), (7, 3, 4), (3, 2, 5)])
+def test_vertex_enumeration_optimum_duality_and_complementarity(n, m, seed):
+    lp = tiny.small_random(n, m, seed)
+    best, xbest = vertex_enumeration(lp)
+    assert np.isfinite(best)
+    for pre in (dict(), dict(ruiz_iters=0, pc_alpha=0.0)):          # scaled and unscaled problem: same optimum
+        s = oracle.solve(lp, eps_rel=1e-8, eps_abs=1e-8, iter_limit=400000, **pre)
+        assert s.status == 0
+        assert abs(s.primal_obj - best) <= 1e-6 * (1 + abs(best))
+        assert abs(s.primal_obj - s.dual_obj) <= 1e-6 * (1 + abs(best))             # strong duality
+        k = dense_kkt(lp, s.x, s.y)                                                 # independent numpy KKT
+        assert k["rp"] <= 1e-6 and k["rd"] <= 1e-6
+        assert k["pobj"] == pytest.approx(s.primal_obj, rel=1e-9, abs=1e-9)
+        assert k["dobj"] == pytest.approx(s.dual_obj, rel=1e-9, abs=1e-9)
+        G = lp.sense == ord("G")
+        assert np.all(s.y[G] >= 0)
+        assert np.abs(s.y * k["slack"]).max() <= 1e-5                               # y_i (Kx-q)_i = 0
+        comp = np.where(k["lam"] > 0, k["lam"] * (s.x - np.where(np.isfinite(lp.l), lp.l, 0)),
+                        k["lam"] * (s.x - np.where(np.isfinite(lp.u), lp.u, 0)))
+        assert np.abs(comp).max() <= 1e-5                                           # lam_j (x_j - bound) = 0
+
+
+def test_termination_measure_at_exact_optimum_and_under_perturbation():
+    lp = tiny.two_var()
+    k = oracle.kkt_unscaled(lp, np.array([1.0, 3.0]), np.array([1.0]))
+    assert k["rel_kkt"] <= 1e-12 and k["pobj"] == -7.0 and k["dobj"] == -7.0
+    # move x1 by +0.5: row -x1-x2 >= -4 violated by exactly 0.5; objective moves by -0.5
+    k = oracle.kkt_unscaled(lp, np.array([1.5, 3.0]), np.array([1.0]))
+    assert k["rp"] == pytest.approx(0.5, rel=1e-15) and k["rd"] == 0.0 and k["pobj"] == -7.5
+    # move y by +0.25: rho = c + y = (-0.75+..): x1 has rho=-1+1.25=0.25>0 with finite lower bound -> lam, no residual
+    k = oracle.kkt_unscaled(lp, np.array([1.0, 3.0]), np.array([1.25]))
+    assert k["rd"] == 0.0 and k["dobj"] == pytest.approx(-4 * 1.25 + 3 * (-2 + 1.25), rel=1e-15)
+    # a free variable turns the same reduced cost into a dual residual
+    lp2 = tiny.free_var_lp()
+    k = oracle.kkt_unscaled(lp2, np.array([1.0, 0.0, 1.0]), np.array([1.0, 0.75]))
+    assert k["rd"] == pytest.approx(0.25, rel=1e-15)
+    for seed in (0, 1):
+        lp3 = tiny.small_random(6, 4, seed)
+        s = oracle.solve(lp3, eps_rel=1e-9, eps_abs=1e-9)
+        a, b = oracle.kkt_unscaled(lp3, s.x, s.y), dense_kkt(lp3, s.x, s.y)
+        for key in ("rp", "rd", "pobj", "dobj"):
+            assert a[key] == pytest.approx(b[key], rel=1e-12, abs=1e-14)
+        # the solver's own (scaled-space) report equals the unscaled definition: identities of R1
+        assert s.primal_obj == pytest.approx(a["pobj"], rel=1e-12, abs=1e-13)
+        assert s.dual_obj == pytest.approx(a["dobj"], rel=1e-12, abs=1e-13)
+        assert s.rel_kkt == pytest.approx(a["rel_kkt"], rel=1e-6, abs=1e-15)
+
+
+# ------------------------------------------------------------------ textbook PDHG properties
+def test_fejer_monotonicity_with_frozen_step():
+    """With restarts off and a constant eta < 1/sigma_max(K), the PDHG-metric distance to a saddle point
+    omega|x-x*|^2 + |y-y*|^2/omega + 2 eta (y-y*)'K(x-x*) never increases (Chambolle-Pock)."""
+    lp = tiny.small_random(6, 4, 2)
+    obj, xs, ys = highs(lp)
+    k = dense_kkt(lp, xs, ys)
+    assert k["rp"] < 1e-9 and k["rd"] < 1e-9 and abs(k["pobj"] - k["dobj"]) < 1e-8     # (x*, y*) is a saddle point
+    K = lp.dense()
+    eta = 0.9 / np.linalg.svd(K, compute_uv=False)[0]
+    N = 300
+    s = oracle.solve(lp, fixed_iterations=N, ruiz_iters=0, pc_alpha=0.0, frozen_eta=eta,
+                     restarts_enabled=0, dump=N, trace_attempts=N)
+    omega = s.omega                       # constant: no restart ever happens
+    assert np.all(s.attempts["accepted"] == 1) and np.all(s.attempts["eta_used"] == eta)
+    ex = s.dump_x - xs; ey = s.dump_y - ys
+    d = omega * (ex ** 2).sum(1) + (ey ** 2).sum(1) / omega + 2 * eta * np.einsum("ki,ij,kj->k", ey, K, ex)
+    assert np.all(d >= -1e-12)
+    assert np.all(np.diff(d) <= 1e-12 * (1 + d[:-1]))
+    assert d[-1] < 0.5 * d[0]
+
+
+def test_average_is_eta_weighted_mean_of_accepted_iterates():
+    lp = tiny.small_random(5, 4, 1)
+    N = 60                                 # < check_every: no restart can clear the sums
+    s = oracle.solve(lp, fixed_iterations=N, dump=N, trace_attempts=N)
+    acc = s.attempts["accepted"] == 1
+    w = s.attempts["eta_used"][acc]
+    assert s.avg_w == pytest.approx(w.sum(), rel=1e-14)
+    np.testing.assert_allclose(s.avg_x, (w[:, None] * s.dump_x[acc]).sum(0) / w.sum(), rtol=1e-12, atol=1e-14)
+    np.testing.assert_allclose(s.avg_y, (w[:, None] * s.dump_y[acc]).sum(0) / w.sum(), rtol=1e-12, atol=1e-14)
+    # rejected attempts leave the iterate untouched (1x1 example rejects attempt 3)
+    s1 = oracle.solve(tiny.one_by_one(), fixed_iterations=4, ruiz_iters=0, pc_alpha=0.0, dump=4, trace_attempts=4)
+    assert s1.attempts["accepted"][2] == 0
+    assert s1.dump_x[2, 0] == s1.dump_x[1, 0] and s1.dump_y[2, 0] == s1.dump_y[1, 0]
+    assert s1.accepted == 3 and s1.iterations == 4
+
+
+# ------------------------------------------------------------------ R10/R11 invariants (decisions unpinned)
+def test_restart_and_primal_weight_invariants():
+    lp = uc_config(0)
+    s = oracle.solve(lp, fixed_iterations=640)
+    assert len(s.checks) == 10 and s.checks["k"].tolist() == [64 * i for i in range(1, 11)]
+    assert s.checks["restart_kind"][0] == 3            # t = k at the first check: artificial restart fires
+    assert np.all(np.isfinite(s.checks["omega_after"])) and np.all(s.checks["omega_after"] > 0)
+    assert s.restarts == int((s.checks["restart_kind"][:-1] > 0).sum()) + int(s.checks["restart_kind"][-1] > 0)
+    # no restart when disabled; omega then never changes
+    s2 = oracle.solve(lp, fixed_iterations=256, restarts_enabled=0)
+    assert s2.restarts == 0 and np.all(s2.checks["restart_kind"] == 0)
+    assert np.all(s2.checks["omega_after"] == s2.checks["omega_after"][0])
+    # after a restart at k=64 the weighted sums restart: with F=64+1 the average holds one iterate
+    s3 = oracle.solve(lp, fixed_iterations=65, trace_attempts=65, dump=65)
+    assert s3.avg_w == pytest.approx(s3.attempts["eta_used"][64], rel=1e-15)
+    np.testing.assert_allclose(s3.avg_x, s3.dump_x[64], rtol=1e-13, atol=1e-300)
+    # box-only LP: y-space is empty so Delta_y = 0 <= 1e-10 and omega must stay at its initial value 1
+    s4 = oracle.solve(tiny.box_only(5, 2), fixed_iterations=200)
+    assert np.all(s4.checks["omega_after"] == 1.0)
+
+
+def test_status_codes_and_iteration_accounting():
+    lp = uc_config(0)
+    s = oracle.solve(lp, iter_limit=100)
+    assert s.status == 1 and s.iterations == 100 and len(s.checks) == 2           # checks at 64 and at the cap
+    s = oracle.solve(lp, fixed_iterations=200, trace_attempts=200)
+    assert s.iterations == 200 and len(s.attempts) == 200 and s.accepted == int(s.attempts["accepted"].sum())
+    assert len(s.checks) == 3 and s.returned_average == 0
+
+
+# ------------------------------------------------------------------ library cross-check on the UC LP
+def test_uc_config0_converges_to_highs_objective():
+    lp = uc_config(0)
+    obj, xh, yh = highs(lp)
+    s = oracle.solve(lp)
+    assert s.status == 0 and s.rel_kkt <= 1e-4
+    assert abs(s.primal_obj - obj) <= 1e-3 * (1 + abs(obj))
+    k = oracle.kkt_unscaled(lp, s.x, s.y)
+    assert k["rel_kkt"] == pytest.approx(s.rel_kkt, rel=1e-6)
+    # HiGHS's own primal-dual pair is optimal under the oracle's KKT definition (sign convention pin)
+    kh = oracle.kkt_unscaled(lp, xh, yh)
+    assert kh["rel_kkt"] <= 1e-7
+    # tighter tolerance moves the objective closer
+    s2 = oracle.solve(lp, eps_rel=1e-7, eps_abs=1e-7, iter_limit=400000)
+    assert s2.status == 0 and abs(s2.primal_obj - obj) <= 1e-5 * (1 + abs(obj))
+
+
+def test_fixed_commitment_objective_not_below_relaxed():
+    """north_star: 'commitment relaxed to [0,1] or fixed' -- fixing u to a 0/1 pattern (l_j = u_j)."""
+    lp = uc_config(0)
+    G, T, V, oU = lp.meta["G"], lp.meta["T"], lp.meta["V"], lp.meta["offsets"]["u"]
+    relaxed = oracle.solve(lp)
+    pattern = (relaxed.x.reshape(T, V)[:, oU:oU + G].T > 0.5).astype(float)
+    lpf = fix_commitment(lp, pattern)
+    obj, _, _ = highs(lpf)                       # feasible for this pattern (HiGHS asserts optimal)
+    fixed = oracle.solve(lpf)
+    assert fixed.status == 0
+    assert fixed.primal_obj >= relaxed.primal_obj * (1 - 1e-3)
+    assert abs(fixed.primal_obj - obj) <= 1e-3 * (1 + abs(obj))
+    np.testing.assert_allclose(fixed.x.reshape(T, V)[:, oU:oU + G].T, pattern, rtol=0, atol=1e-14)   # clamp keeps l = u
+
+
+def test_warm_start_from_solution_terminates_at_first_check():
+    lp = tiny.small_random(6, 4, 0)
+    s = oracle.solve(lp, eps_rel=1e-9, eps_abs=1e-9)
+    s2 = oracle.solve(lp, x0=s.x, y0=s.y, eps_rel=1e-6, eps_abs=1e-6)
+    assert s2.status == 0 and s2.iterations == 64
