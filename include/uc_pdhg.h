@@ -1,0 +1,194 @@
+/*
+ * uc_pdhg.h -- C ABI of the B200-native restarted PDHG (PDLP-style) LP solver.
+ *
+ * What it solves (BASELINE.json north_star; "One solver employs the PDHG algorithm to
+ * solve the relaxed linear problem using a GPU"):
+ *
+ *        min c'x   s.t.   (A x)_i = b_i  (sense 'E')  or  (A x)_i >= b_i  (sense 'G'),   l <= x <= u
+ *
+ * i.e. the LP relaxation of the DC unit-commitment MILP (commitment relaxed to [0,1], or fixed by
+ * l = u).  The algorithm is fixed step by step in DESIGN.md "Readings" R1..R14 (SURVEY.md 8(c)
+ * O0..O7): Ruiz + Pock-Chambolle diagonal preconditioning, adaptive-step PDHG with the
+ * extrapolation 2x+ - x, eta-weighted averaging, KKT-based restarts, primal-weight update,
+ * relative-KKT termination.  Default stopping parameters are the paper's (PAPER.md l.66, l.91:
+ * iteration limit 100,000; convergence tolerance 1e-4; absolute feasibility tolerance 1e-5 opt-in).
+ * uc_pdhg_cancel is the hook for Algorithm 1: "Terminate the other solver".
+ *
+ * Conventions
+ *   - every call returns 0 on success, or a negative uc_error; no exception or abort crosses the ABI;
+ *     uc_last_error() returns the text of the last failure on this thread.
+ *   - all array arguments are HOST pointers unless the name says `_device`; the library copies
+ *     what it needs; the caller keeps ownership of everything it passes in.
+ *   - all device memory, streams, events and CUDA graphs are owned by the handle and released
+ *     by uc_lp_destroy.  The handle is bound to one device.
+ *   - there is no CPU fallback: every call that computes fails with UC_ERR_CUDA without a GPU.
+ *   - dual sign convention: Lagrangian c'x - y'(A x - b), so y_i >= 0 on 'G' rows.
+ *   - uc_pdhg_solve* is blocking and not re-entrant per handle; uc_pdhg_cancel may be called
+ *     from any thread at any time.
+ */
+#ifndef UC_PDHG_H
+#define UC_PDHG_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct uc_lp uc_lp; /* opaque */
+
+enum uc_error {
+    UC_OK = 0,
+    UC_ERR_INVALID = -1, /* bad argument (NULL, negative size, column out of range, duplicate entry, l > u, NaN) */
+    UC_ERR_CUDA = -2,    /* a CUDA runtime call or kernel failed (includes: no device) */
+    UC_ERR_NOMEM = -3,   /* host or device allocation failed */
+    UC_ERR_BUSY = -4     /* a solve is already running on this handle */
+};
+
+enum uc_status {
+    UC_OPTIMAL = 0,         /* relative KKT test passed (R12) */
+    UC_ITERATION_LIMIT = 1, /* iter_limit attempts done (also the status of every fixed_iterations run) */
+    UC_CANCELLED = 2,       /* uc_pdhg_cancel was seen */
+    UC_TIME_LIMIT = 3,
+    UC_NUMERICAL_ERROR = 4  /* a non-finite step size or KKT term appeared */
+};
+
+/* ------------------------------------------------------------------------------------------ create */
+typedef struct {
+    int32_t device;             /* CUDA device ordinal; -1 = current device */
+    int32_t ruiz_iters;         /* 10  (R1) */
+    double pc_alpha;            /* 1.0; 0 = no Pock-Chambolle pass (R1) */
+    int32_t sell_window;        /* rows per length-sorting window of the sliced-ELL layout; 4096 */
+    int32_t long_row_threshold; /* rows longer than this leave the sliced-ELL part (warp-per-row); 32 */
+    int32_t keep_source_map;    /* 1: keep the slot -> CSR position maps on the host (uc_lp_get_scaled_values); 0 */
+    int32_t pad_;
+} uc_lp_options;
+
+void uc_lp_default_options(uc_lp_options* opt);
+
+/*
+ * Ingest + transpose + preconditioning.
+ *   m, n, nnz        rows, columns, nonzeros (any may be 0)
+ *   row_ptr[m+1]     CSR row pointers, row_ptr[0] = 0, row_ptr[m] = nnz
+ *   col_idx[nnz]     0-based column indices; order inside a row is free; duplicates are an error
+ *   val[nnz]         finite values
+ *   sense[m]         'E' or 'G'
+ *   b[m], c[n]       finite;  l[n], u[n]: l <= u, -INFINITY / +INFINITY or |v| >= 1e20 = absent (R13)
+ *   opt              NULL = defaults
+ *   out              receives the handle
+ */
+int uc_lp_create(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, const int32_t* col_idx,
+                 const double* val, const char* sense, const double* b, const double* c, const double* l,
+                 const double* u, const uc_lp_options* opt, uc_lp** out);
+
+/* Replace the bounds (fixed-commitment re-solves, north_star "relaxed to [0,1] or fixed"); the
+   matrix, its scalings and the captured graph are kept.  l_new/u_new: host, length n. */
+int uc_lp_update_bounds(uc_lp* lp, const double* l_new, const double* u_new);
+
+void uc_lp_destroy(uc_lp* lp); /* NULL ok; must not race with a solve on the same handle */
+
+/* ------------------------------------------------------------------------------------------- solve */
+/* per-attempt trace record (R5): step size used, the bound eta_bar, the next step size, the three
+   reductions, and whether the attempt was accepted */
+typedef struct {
+    double eta_used, eta_bar, eta_next, dx2, dy2, inter;
+    int32_t accepted, pad_;
+} uc_attempt_record;
+
+/* per-check trace record (R8..R11) */
+typedef struct {
+    int64_t k;
+    int32_t restart_kind; /* 0 none, 1 sufficient, 2 necessary, 3 artificial */
+    int32_t candidate;    /* 0 current, 1 average */
+    double omega_after, mu_c, mu_r, relkkt_cur, relkkt_avg;
+} uc_check_record;
+
+typedef struct {
+    int64_t iter_limit;       /* 100000 */
+    double eps_rel;           /* 1e-4    PAPER.md l.91 "convergence tolerance" */
+    double eps_abs;           /* 1e-4 (= eps_rel, R12); 1e-5 reproduces the paper's extra knob (l.66) */
+    double time_limit_s;      /* +inf */
+    int32_t check_every;      /* 64 (R8) */
+    int32_t pad_;
+    int64_t fixed_iterations; /* 0 = off; F > 0: exactly F attempts, termination test off, current iterate returned (R14) */
+    double beta_sufficient;   /* 0.2  (R10) */
+    double beta_necessary;    /* 0.8  (R10) */
+    double beta_artificial;   /* 0.36 (R10) */
+    double weight_smoothing;  /* 0.5  (R11) */
+    const double* x0;         /* nullable warm start, original space, length n (host; `_device` call: device) */
+    const double* y0;         /* nullable warm start, original space, length m */
+    void* stream;             /* cudaStream_t to run on; NULL = the handle's own stream */
+    uc_attempt_record* attempt_trace; /* nullable HOST buffer, attempt_trace_cap records */
+    int64_t attempt_trace_cap;
+    uc_check_record* check_trace;     /* nullable HOST buffer, check_trace_cap records */
+    int64_t check_trace_cap;
+} uc_pdhg_params;
+
+void uc_pdhg_default_params(uc_pdhg_params* p);
+
+typedef struct {
+    int32_t status;           /* enum uc_status */
+    int32_t returned_average; /* 1 if x, y are the averaged iterate */
+    int64_t iterations;       /* attempts (each = one K' pass + one K pass, accepted or not) */
+    int64_t accepted, restarts;
+    double rel_kkt, rel_primal_res, rel_dual_res, rel_gap, primal_obj, dual_obj;
+    double eta, omega;        /* final step size and primal weight */
+    double solve_seconds;     /* host wall clock of this call */
+    double loop_seconds;      /* device time (CUDA events) of the attempt loop incl. checks */
+    int64_t attempt_records, check_records; /* records produced (may exceed the capacities given) */
+    int64_t kernel_launches;  /* kernels of this library executed by the call (graph nodes included) */
+} uc_pdhg_result;
+
+/* Run restarted PDHG.  x_out[n], y_out[m]: HOST buffers receiving the returned point in the
+   original space (nullable).  params NULL = defaults. */
+int uc_pdhg_solve(uc_lp* lp, const uc_pdhg_params* params, double* x_out, double* y_out, uc_pdhg_result* result);
+
+/* Same, with x_out / y_out / params->x0 / params->y0 being DEVICE pointers on the handle's device
+   (the torch harness owns them); nothing but the result struct and the traces crosses PCIe. */
+int uc_pdhg_solve_device(uc_lp* lp, const uc_pdhg_params* params, double* x_out_device, double* y_out_device,
+                         uc_pdhg_result* result);
+
+/* Sticky cancel flag, any thread, idempotent.  A solve that finds it set -- at entry or at any
+   check -- returns UC_CANCELLED and clears it, so a cancel that lands just before the solve starts
+   is not lost (the race of Algorithm 1). */
+int uc_pdhg_cancel(uc_lp* lp);
+
+/* ------------------------------------------------------------------------------- introspection */
+typedef struct {
+    int64_t m, n, nnz;
+    int64_t k_sell_slots, kt_sell_slots; /* stored slots (incl. padding) of the sliced-ELL parts */
+    int64_t k_long_rows, kt_long_rows;   /* rows handled warp-per-row */
+    int64_t k_long_nnz, kt_long_nnz;
+    int64_t device_bytes;                /* device memory owned by the handle */
+    double precondition_seconds;         /* device time of A2..A4 */
+    double create_seconds;               /* host wall clock of uc_lp_create */
+    double eta0, omega0;                 /* R2 */
+    double norm_b, norm_c;               /* unscaled 2-norms used by R9 */
+    int64_t bytes_per_attempt;           /* bytes one attempt streams in this layout */
+} uc_lp_info;
+
+int uc_lp_get_info(const uc_lp* lp, uc_lp_info* info);
+
+/* Diagonal scalings of R1, original row/column order: K = diag(Dr) Ktilde diag(Dc).  HOST out. */
+int uc_lp_get_scaling(uc_lp* lp, double* Dr_out, double* Dc_out);
+
+/* Scaled matrix values Ktilde in the caller's CSR order (val_out[nnz]) read back from the K layout
+   (from_transpose = 0) or from the explicit K' layout (from_transpose = 1).  HOST out.  Test hook
+   for R1 and for "K' equals the CSC of K bit-exactly". */
+int uc_lp_get_scaled_values(uc_lp* lp, int32_t from_transpose, double* val_out);
+
+/* out = Ktilde v (transpose = 0; v[n], out[m]) or Ktilde' v (transpose = 1; v[m], out[n]) with the
+   solver's own SpMV kernels; HOST in/out, original order.  Test hook for the adjoint identity. */
+int uc_lp_spmv(uc_lp* lp, int32_t transpose, const double* v, double* out);
+
+/* Host evaluation of the double-double log / exp that the primal-weight update (R11) runs on the
+   device (same source, csrc/uc_dd.cuh).  Test hooks: no GPU needed. */
+double uc_host_log_rounded(double a);
+double uc_host_exp_rounded(double x);
+
+const char* uc_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* UC_PDHG_H */

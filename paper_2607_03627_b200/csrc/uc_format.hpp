@@ -1,0 +1,172 @@
+// uc_format.hpp -- host-side ingest: validation, transpose and the sliced-ELL layout.
+//
+// Layout ("SELL-32 + long tail"):
+//   rows are relabelled  new -> old  by `perm`:  rows with at most `long_thr` entries come first,
+//   taken in the caller's order in windows of `window` rows and sorted by length inside each window
+//   (stable counting sort), so that 32 consecutive rows -- one slice, one warp -- have (nearly) equal
+//   length; rows longer than `long_thr` follow and are stored as plain CSR (one warp per row).
+//   Slice s holds rows 32s..32s+31 column-major: slot(base_s + t*32 + lane) = t-th entry of row
+//   32s+lane, padded with (col 0, val 0) up to the slice width, so lane-consecutive loads coalesce.
+// The relabelling is internal: both matrices, all vectors and both diagonal scalings live in the
+// permuted index spaces; results are un-permuted on the way out.
+#pragma once
+#include <cstdint>
+#include <string>
+#include <vector>
+#include <algorithm>
+#include <cmath>
+
+namespace ucpdhg {
+
+struct HostSell {
+    int64_t nrows = 0, nshort = 0, nlong = 0, nslices = 0;
+    std::vector<int64_t> slice_ptr;   // [nslices+1]
+    std::vector<int32_t> col;         // [slots]
+    std::vector<double> val;          // [slots]
+    std::vector<int64_t> src;         // [slots]  caller's CSR position of the slot, -1 = padding (only if asked for)
+    std::vector<int64_t> lptr;        // [nlong+1]
+    std::vector<int32_t> lcol;
+    std::vector<double> lval;
+    std::vector<int64_t> lsrc;
+};
+
+// new -> old permutation: short rows in length-sorted windows, long rows last.
+inline void build_perm(const std::vector<int64_t>& len, int64_t window, int64_t long_thr,
+                       std::vector<int64_t>& perm, std::vector<int64_t>& inv, int64_t& nshort) {
+    const int64_t N = (int64_t)len.size();
+    perm.clear(); perm.reserve(N);
+    std::vector<int64_t> longs, win;
+    std::vector<int64_t> cnt((size_t)long_thr + 2);
+    win.reserve((size_t)window);
+    auto flush = [&]() {
+        std::fill(cnt.begin(), cnt.end(), 0);
+        for (int64_t r : win) cnt[(size_t)len[r] + 1]++;
+        for (size_t k = 1; k < cnt.size(); ++k) cnt[k] += cnt[k - 1];
+        size_t base = perm.size();
+        perm.resize(base + win.size());
+        for (int64_t r : win) perm[base + (size_t)cnt[(size_t)len[r]]++] = r;
+        win.clear();
+    };
+    for (int64_t r = 0; r < N; ++r) {
+        if (len[r] > long_thr) { longs.push_back(r); continue; }
+        win.push_back(r);
+        if ((int64_t)win.size() == window) flush();
+    }
+    if (!win.empty()) flush();
+    nshort = (int64_t)perm.size();
+    perm.insert(perm.end(), longs.begin(), longs.end());
+    inv.assign((size_t)N, 0);
+    for (int64_t k = 0; k < N; ++k) inv[(size_t)perm[k]] = k;
+}
+
+// CSR (ptr, idx, val, optional src positions) with rows relabelled by perm and column indices by
+// inv_other -> SELL + long tail.
+inline void build_sell(int64_t nrows, const int64_t* ptr, const int32_t* idx, const double* val, const int64_t* srcpos,
+                       const std::vector<int64_t>& perm, int64_t nshort, const std::vector<int64_t>& inv_other,
+                       bool want_src, HostSell& S) {
+    S.nrows = nrows; S.nshort = nshort; S.nlong = nrows - nshort;
+    S.nslices = (nshort + 31) / 32;
+    S.slice_ptr.assign((size_t)S.nslices + 1, 0);
+    for (int64_t s = 0; s < S.nslices; ++s) {
+        int64_t w = 0;
+        for (int64_t r = 32 * s; r < std::min<int64_t>(32 * s + 32, nshort); ++r) {
+            int64_t o = perm[(size_t)r];
+            w = std::max(w, ptr[o + 1] - ptr[o]);
+        }
+        S.slice_ptr[(size_t)s + 1] = S.slice_ptr[(size_t)s] + 32 * w;
+    }
+    const int64_t slots = S.slice_ptr[(size_t)S.nslices];
+    S.col.assign((size_t)slots, 0); S.val.assign((size_t)slots, 0.0);
+    if (want_src) S.src.assign((size_t)slots, -1);
+    for (int64_t r = 0; r < nshort; ++r) {
+        int64_t o = perm[(size_t)r], s = r >> 5, lane = r & 31, base = S.slice_ptr[(size_t)s];
+        for (int64_t p = ptr[o], t = 0; p < ptr[o + 1]; ++p, ++t) {
+            size_t k = (size_t)(base + t * 32 + lane);
+            S.col[k] = (int32_t)inv_other[(size_t)idx[p]];
+            S.val[k] = val[p];
+            if (want_src) S.src[k] = srcpos ? srcpos[p] : p;
+        }
+    }
+    S.lptr.assign((size_t)S.nlong + 1, 0);
+    for (int64_t r = 0; r < S.nlong; ++r) {
+        int64_t o = perm[(size_t)(nshort + r)];
+        S.lptr[(size_t)r + 1] = S.lptr[(size_t)r] + (ptr[o + 1] - ptr[o]);
+    }
+    const int64_t lnnz = S.lptr[(size_t)S.nlong];
+    S.lcol.resize((size_t)lnnz); S.lval.resize((size_t)lnnz);
+    if (want_src) S.lsrc.resize((size_t)lnnz);
+    for (int64_t r = 0; r < S.nlong; ++r) {
+        int64_t o = perm[(size_t)(nshort + r)], k = S.lptr[(size_t)r];
+        for (int64_t p = ptr[o]; p < ptr[o + 1]; ++p, ++k) {
+            S.lcol[(size_t)k] = (int32_t)inv_other[(size_t)idx[p]];
+            S.lval[(size_t)k] = val[p];
+            if (want_src) S.lsrc[(size_t)k] = srcpos ? srcpos[p] : p;
+        }
+    }
+}
+
+struct HostProblem {
+    int64_t m = 0, n = 0, nnz = 0;
+    std::vector<int64_t> perm_r, inv_r, perm_c, inv_c;   // new -> old, old -> new
+    HostSell K, KT;
+};
+
+// Validate the caller's CSR (A0) and return "" or the reason it is rejected.
+inline std::string validate_csr(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, const int32_t* col_idx,
+                                const double* val, const char* sense, const double* b, const double* c,
+                                const double* l, const double* u) {
+    if (m < 0 || n < 0 || nnz < 0) return "negative size";
+    if (!row_ptr) return "row_ptr is NULL";
+    if (m > 2000000000LL || n > 2000000000LL || nnz > 2000000000LL) return "size exceeds the int32 index range of the layout";
+    if (row_ptr[0] != 0 || row_ptr[m] != nnz) return "row_ptr[0] != 0 or row_ptr[m] != nnz";
+    if (nnz > 0 && (!col_idx || !val)) return "col_idx / val is NULL";
+    if ((m > 0 && (!sense || !b)) || (n > 0 && (!c || !l || !u))) return "a vector argument is NULL";
+    std::vector<int64_t> stamp((size_t)std::max<int64_t>(n, 1), -1);
+    for (int64_t i = 0; i < m; ++i) {
+        if (row_ptr[i + 1] < row_ptr[i]) return "row_ptr is not monotone";
+        if (sense[i] != 'E' && sense[i] != 'G') return "sense must be 'E' or 'G'";
+        if (!std::isfinite(b[i])) return "b has a non-finite entry";
+        for (int64_t p = row_ptr[i]; p < row_ptr[i + 1]; ++p) {
+            int64_t j = col_idx[p];
+            if (j < 0 || j >= n) return "column index out of range";
+            if (stamp[(size_t)j] == i) return "duplicate entry within a row";
+            stamp[(size_t)j] = i;
+            if (!std::isfinite(val[p])) return "val has a non-finite entry";
+        }
+    }
+    for (int64_t j = 0; j < n; ++j) {
+        if (!std::isfinite(c[j])) return "c has a non-finite entry";
+        if (std::isnan(l[j]) || std::isnan(u[j])) return "a bound is NaN";
+        if (l[j] > u[j]) return "l > u";
+    }
+    return "";
+}
+
+// A1: explicit transpose (counting sort by column, stable in the row index) + both SELL layouts.
+inline void build_problem(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, const int32_t* col_idx,
+                          const double* val, int64_t window, int64_t long_thr, bool want_src, HostProblem& P) {
+    P.m = m; P.n = n; P.nnz = nnz;
+    std::vector<int64_t> lenr((size_t)m), lenc((size_t)n, 0);
+    for (int64_t i = 0; i < m; ++i) lenr[(size_t)i] = row_ptr[i + 1] - row_ptr[i];
+    for (int64_t p = 0; p < nnz; ++p) lenc[(size_t)col_idx[p]]++;
+    int64_t ms = 0, ns = 0;
+    build_perm(lenr, window, long_thr, P.perm_r, P.inv_r, ms);
+    build_perm(lenc, window, long_thr, P.perm_c, P.inv_c, ns);
+    build_sell(m, row_ptr, col_idx, val, nullptr, P.perm_r, ms, P.inv_c, want_src, P.K);
+    // transpose
+    std::vector<int64_t> tptr((size_t)n + 1, 0), tsrc((size_t)nnz);
+    std::vector<int32_t> tidx((size_t)nnz);
+    std::vector<double> tval((size_t)nnz);
+    for (int64_t j = 0; j < n; ++j) tptr[(size_t)j + 1] = tptr[(size_t)j] + lenc[(size_t)j];
+    {
+        std::vector<int64_t> fill(tptr.begin(), tptr.end() - 1);
+        for (int64_t i = 0; i < m; ++i)
+            for (int64_t p = row_ptr[i]; p < row_ptr[i + 1]; ++p) {
+                int64_t k = fill[(size_t)col_idx[p]]++;
+                tidx[(size_t)k] = (int32_t)i; tval[(size_t)k] = val[p]; tsrc[(size_t)k] = p;
+            }
+    }
+    build_sell(n, tptr.data(), tidx.data(), tval.data(), tsrc.data(), P.perm_c, ns, P.inv_r, want_src, P.KT);
+}
+
+}  // namespace ucpdhg

@@ -1,0 +1,629 @@
+// uc_pdhg.cu -- the C ABI of include/uc_pdhg.h: handle, ingest, preconditioning driver, the
+// CUDA-graph iteration loop, cancel, output.  All arithmetic of the method runs in the kernels of
+// uc_kernels.cuh; the host only marshals, launches and polls.  There is no CPU fallback.
+#include <atomic>
+#include <chrono>
+#include <cstdio>
+#include <cstring>
+#include <limits>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "uc_format.hpp"
+#include "uc_kernels.cuh"
+
+using namespace ucpdhg;
+
+namespace {
+
+thread_local std::string g_err;
+
+int fail(int code, const std::string& msg) { g_err = msg; return code; }
+
+struct CudaFail { cudaError_t e; const char* what; };
+#define CK(call)                                                 \
+    do {                                                         \
+        cudaError_t e__ = (call);                                \
+        if (e__ != cudaSuccess) throw CudaFail{e__, #call};      \
+    } while (0)
+
+double now_s() {
+    return std::chrono::duration<double>(std::chrono::steady_clock::now().time_since_epoch()).count();
+}
+inline int cdiv(long long a, long long b) { return (int)((a + b - 1) / b); }
+
+}  // namespace
+
+struct uc_lp {
+    int device = 0;
+    cudaStream_t own_stream = nullptr;
+    int64_t m = 0, n = 0, nnz = 0;
+    uc_lp_options opt{};
+    std::vector<void*> allocs;
+    size_t device_bytes = 0;
+    // permutations (device, new -> old)
+    long long *perm_r = nullptr, *perm_c = nullptr;
+    Sell K{}, KT{};
+    Vecs V{};
+    Ctrl* ctl = nullptr;
+    double *Dr = nullptr, *Dc = nullptr;   // writable aliases of V.Dr / V.Dc
+    double *qs = nullptr, *cs = nullptr, *ls = nullptr, *us = nullptr;
+    unsigned char* isG = nullptr;
+    // host <-> device mailboxes (pinned, mapped)
+    HostStatus* h_status = nullptr; HostStatus* d_status = nullptr;
+    int* h_stop = nullptr; int* d_stop = nullptr;
+    std::atomic<int> cancel_requested{0};
+    std::atomic<int> busy{0};
+    // one-time scalars
+    double eta0 = 1.0, omega0 = 1.0, norm_b = 0.0, norm_c = 0.0;
+    double precondition_seconds = 0.0, create_seconds = 0.0;
+    int64_t k_slots = 0, kt_slots = 0, k_long_nnz = 0, kt_long_nnz = 0;
+    // step-rule factors {(k+1)^-0.6, (k+1)^-0.3}, k = 1.. (R5): a constant schedule, tabulated once
+    double2* powtab = nullptr;
+    long long powtab_len = 0;
+    // graph cache
+    cudaGraphExec_t exec = nullptr;
+    int graph_ce = 0;
+    int graph_nodes = 0;
+    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+    cudaEvent_t ev_t0 = nullptr, ev_t1 = nullptr;
+    // source maps for uc_lp_get_scaled_values (only with keep_source_map)
+    std::vector<int64_t> k_src, k_lsrc, kt_src, kt_lsrc;
+    // host permutations (for warm starts / hooks)
+    std::vector<int64_t> h_perm_r, h_perm_c;
+
+    template <class T>
+    T* dalloc(size_t count) {
+        void* p = nullptr;
+        size_t bytes = (count ? count : 1) * sizeof(T);
+        cudaError_t e = cudaMalloc(&p, bytes);
+        if (e != cudaSuccess) throw CudaFail{e, "cudaMalloc"};
+        allocs.push_back(p);
+        device_bytes += bytes;
+        return (T*)p;
+    }
+    template <class T>
+    T* upload(const std::vector<T>& h) {
+        T* d = dalloc<T>(h.size());
+        if (!h.empty()) CK(cudaMemcpy(d, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice));
+        return d;
+    }
+};
+
+namespace {
+
+struct DeviceGuard {
+    int prev = -1;
+    explicit DeviceGuard(int dev) { cudaGetDevice(&prev); if (prev != dev) cudaSetDevice(dev); else prev = -1; }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+Sell upload_sell(uc_lp* lp, const HostSell& H) {
+    Sell S{};
+    static_assert(sizeof(long long) == sizeof(int64_t), "int64 layout");
+    S.sp = (const long long*)lp->upload(H.slice_ptr);
+    S.col = lp->upload(H.col);
+    S.val = lp->upload(H.val);
+    S.nshort = H.nshort; S.nslices = (int)H.nslices; S.nblk = cdiv(H.nslices, kWarps);
+    S.lp = (const long long*)lp->upload(H.lptr);
+    S.lcol = lp->upload(H.lcol);
+    S.lval = lp->upload(H.lval);
+    S.nlong = (int)H.nlong;
+    S.nlblk = cdiv(H.nlong, kWarps);
+    S.grid = S.nlblk + S.nblk;
+    if (S.grid < 1) S.grid = 1;
+    return S;
+}
+
+// two-stage reduction of a device array to one host double (op 0: sum of squares, 1: max |v|)
+double reduce_to_host(uc_lp* lp, const double* v, long long count, int op, dd* part, double* out_dev, cudaStream_t st) {
+    int blocks = count > 0 ? std::min<long long>(1024, (count + kBlock - 1) / kBlock) : 1;
+    k_reduce<<<blocks, kBlock, 0, st>>>(v, count, op, part);
+    k_reduce_final<<<1, 32, 0, st>>>(part, blocks, op, out_dev);
+    double h = 0.0;
+    CK(cudaMemcpyAsync(&h, out_dev, sizeof(double), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    (void)lp;
+    return h;
+}
+
+// R1: Ruiz x ruiz_iters, then Pock-Chambolle(alpha); accumulates Dr, Dc; scales both layouts.
+void precondition(uc_lp* lp, cudaStream_t st) {
+    const long long m = lp->m, n = lp->n;
+    double* r = lp->dalloc<double>((size_t)m);
+    double* s = lp->dalloc<double>((size_t)n);
+    k_vec_fill<<<cdiv(std::max<long long>(m, 1), 256), 256, 0, st>>>(lp->Dr, 1.0, m);
+    k_vec_fill<<<cdiv(std::max<long long>(n, 1), 256), 256, 0, st>>>(lp->Dc, 1.0, n);
+    const double alpha = lp->opt.pc_alpha;
+    const int passes = lp->opt.ruiz_iters + (alpha > 0.0 ? 1 : 0);
+    for (int pass = 0; pass < passes; ++pass) {
+        const bool ruiz = pass < lp->opt.ruiz_iters;
+        int mode_r = ruiz ? 0 : (alpha == 1.0 ? 1 : 2), mode_c = mode_r;
+        double p_r = 2.0 - alpha, p_c = alpha;
+        k_row_stat<<<lp->K.grid, kBlock, 0, st>>>(lp->K, mode_r, p_r, r);
+        k_row_stat<<<lp->KT.grid, kBlock, 0, st>>>(lp->KT, mode_c, p_c, s);
+        k_scale_matrix<<<lp->K.grid, kBlock, 0, st>>>(lp->K, r, s);
+        k_scale_matrix<<<lp->KT.grid, kBlock, 0, st>>>(lp->KT, s, r);
+        k_vec_mul<<<cdiv(std::max<long long>(m, 1), 256), 256, 0, st>>>(lp->Dr, r, m);
+        k_vec_mul<<<cdiv(std::max<long long>(n, 1), 256), 256, 0, st>>>(lp->Dc, s, n);
+    }
+    CK(cudaGetLastError());
+}
+
+// The factors of the step rule depend on the attempt counter only.  They are tabulated on the host with
+// the C library's pow (correctly rounded in all but freak cases), because one ulp in eta is amplified
+// exponentially by the adaptive rule and CUDA's pow is only 2-ulp accurate.
+void ensure_powtab(uc_lp* lp, long long limit) {
+    if (limit <= lp->powtab_len) return;
+    long long len = std::max<long long>(limit, 4096);
+    std::vector<double2> h((size_t)len);
+    for (long long k = 1; k <= len; ++k) h[(size_t)k - 1] = make_double2(std::pow((double)(k + 1), -0.6), std::pow((double)(k + 1), -0.3));
+    if (lp->powtab) { cudaFree(lp->powtab); lp->powtab = nullptr; lp->powtab_len = 0; }
+    CK(cudaMalloc((void**)&lp->powtab, sizeof(double2) * (size_t)len));
+    CK(cudaMemcpy(lp->powtab, h.data(), sizeof(double2) * (size_t)len, cudaMemcpyHostToDevice));
+    lp->powtab_len = len;
+}
+
+void launch_attempt(uc_lp* lp, cudaStream_t st) {
+    k_primal<<<lp->KT.grid, kBlock, 0, st>>>(lp->KT, lp->V, lp->ctl);
+    k_dual<<<lp->K.grid, kBlock, 0, st>>>(lp->K, lp->V, lp->ctl);
+}
+void launch_kkt(uc_lp* lp, cudaStream_t st, int mode) {
+    k_check_dual<<<lp->KT.grid, kBlock, 0, st>>>(lp->KT, lp->V, lp->ctl);
+    k_check_primal<<<lp->K.grid, kBlock, 0, st>>>(lp->K, lp->V, lp->ctl);
+    k_check_finalize<<<1, kFinalBlock, 0, st>>>(lp->V, lp->ctl, mode);
+}
+void launch_check(uc_lp* lp, cudaStream_t st) {
+    k_flush<<<lp->V.gridR, kBlock, 0, st>>>(lp->V, lp->ctl);
+    launch_kkt(lp, st, kModeCheck);
+    k_restart_vec<<<lp->V.gridR, kBlock, 0, st>>>(lp->V, lp->ctl);
+    k_restart_finalize<<<1, kFinalBlock, 0, st>>>(lp->V, lp->ctl);
+}
+constexpr int kCheckLaunches = 6;
+
+// capture `ce` attempts + one check into an executable graph (A15)
+void build_graph(uc_lp* lp, int ce) {
+    if (lp->exec && lp->graph_ce == ce) return;
+    if (lp->exec) { cudaGraphExecDestroy(lp->exec); lp->exec = nullptr; }
+    cudaGraph_t g = nullptr;
+    CK(cudaStreamBeginCapture(lp->own_stream, cudaStreamCaptureModeThreadLocal));
+    for (int i = 0; i < ce; ++i) launch_attempt(lp, lp->own_stream);
+    launch_check(lp, lp->own_stream);
+    CK(cudaStreamEndCapture(lp->own_stream, &g));
+    CK(cudaGraphInstantiate(&lp->exec, g, 0));
+    CK(cudaGraphDestroy(g));
+    lp->graph_ce = ce;
+    lp->graph_nodes = 2 * ce + kCheckLaunches;
+}
+
+void destroy_impl(uc_lp* lp) {
+    if (!lp) return;
+    cudaSetDevice(lp->device);
+    if (lp->exec) cudaGraphExecDestroy(lp->exec);
+    for (auto& e : lp->ev) if (e) cudaEventDestroy(e);
+    if (lp->ev_t0) cudaEventDestroy(lp->ev_t0);
+    if (lp->ev_t1) cudaEventDestroy(lp->ev_t1);
+    for (void* p : lp->allocs) cudaFree(p);
+    if (lp->powtab) cudaFree(lp->powtab);
+    if (lp->h_status) cudaFreeHost(lp->h_status);
+    if (lp->h_stop) cudaFreeHost(lp->h_stop);
+    if (lp->own_stream) cudaStreamDestroy(lp->own_stream);
+    delete lp;
+}
+
+int64_t bytes_per_attempt(const uc_lp* lp) {
+    // what one attempt streams in THIS layout: matrix slots (12 B each, padding included),
+    // slice pointers, and per variable 8 (x) + 24 (c,l,u) + 16 (xsum r/w) + 8 (x') + 16 ({xbar,dx}) + 16
+    // (gather of the pair) = 88 B, per row 8 (y) + 8 (q) + 1 (sense) + 16 (ysum r/w) + 8 (y') + 8 (gather) = 49 B
+    return 12 * (lp->k_slots + lp->kt_slots + lp->k_long_nnz + lp->kt_long_nnz) + 8 * ((int64_t)lp->K.nslices + lp->KT.nslices) +
+           88 * lp->n + 49 * lp->m;
+}
+
+}  // namespace
+
+// ================================================================================== C ABI
+extern "C" {
+
+const char* uc_last_error(void) { return g_err.c_str(); }
+
+double uc_host_log_rounded(double a) { return log_rounded(a); }
+double uc_host_exp_rounded(double x) { return exp_rounded(x); }
+
+void uc_lp_default_options(uc_lp_options* o) {
+    if (!o) return;
+    o->device = -1; o->ruiz_iters = 10; o->pc_alpha = 1.0; o->sell_window = 4096; o->long_row_threshold = 32;
+    o->keep_source_map = 0; o->pad_ = 0;
+}
+
+void uc_pdhg_default_params(uc_pdhg_params* p) {
+    if (!p) return;
+    std::memset(p, 0, sizeof *p);
+    p->iter_limit = 100000; p->eps_rel = 1e-4; p->eps_abs = 1e-4;
+    p->time_limit_s = std::numeric_limits<double>::infinity();
+    p->check_every = 64; p->fixed_iterations = 0;
+    p->beta_sufficient = 0.2; p->beta_necessary = 0.8; p->beta_artificial = 0.36; p->weight_smoothing = 0.5;
+}
+
+int uc_lp_create(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, const int32_t* col_idx, const double* val,
+                 const char* sense, const double* b, const double* c, const double* l, const double* u,
+                 const uc_lp_options* opt_in, uc_lp** out) {
+    if (!out) return fail(UC_ERR_INVALID, "out is NULL");
+    *out = nullptr;
+    const double t_create = now_s();
+    uc_lp_options opt;
+    uc_lp_default_options(&opt);
+    if (opt_in) opt = *opt_in;
+    if (opt.ruiz_iters < 0 || opt.pc_alpha < 0.0 || opt.pc_alpha > 2.0 || opt.sell_window < 32 || opt.long_row_threshold < 1)
+        return fail(UC_ERR_INVALID, "bad uc_lp_options");
+    std::string why = validate_csr(m, n, nnz, row_ptr, col_idx, val, sense, b, c, l, u);
+    if (!why.empty()) return fail(UC_ERR_INVALID, why);
+
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
+        return fail(UC_ERR_CUDA, "no CUDA device: this library has no CPU path");
+    int dev = opt.device;
+    if (dev < 0) { if (cudaGetDevice(&dev) != cudaSuccess) return fail(UC_ERR_CUDA, "cudaGetDevice failed"); }
+    if (dev >= ndev) return fail(UC_ERR_INVALID, "device ordinal out of range");
+
+    uc_lp* lp = nullptr;
+    try {
+        lp = new uc_lp();
+        lp->device = dev; lp->m = m; lp->n = n; lp->nnz = nnz; lp->opt = opt;
+        DeviceGuard guard(dev);
+        CK(cudaStreamCreateWithFlags(&lp->own_stream, cudaStreamNonBlocking));
+        for (auto& e : lp->ev) CK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        CK(cudaEventCreate(&lp->ev_t0)); CK(cudaEventCreate(&lp->ev_t1));
+        cudaStream_t st = lp->own_stream;
+
+        // A0 / A1: layouts (host), upload
+        HostProblem P;
+        build_problem(m, n, nnz, row_ptr, col_idx, val, opt.sell_window, opt.long_row_threshold, opt.keep_source_map != 0, P);
+        lp->K = upload_sell(lp, P.K);
+        lp->KT = upload_sell(lp, P.KT);
+        lp->k_slots = (int64_t)P.K.col.size(); lp->kt_slots = (int64_t)P.KT.col.size();
+        lp->k_long_nnz = (int64_t)P.K.lcol.size(); lp->kt_long_nnz = (int64_t)P.KT.lcol.size();
+        lp->perm_r = (long long*)lp->upload(P.perm_r);
+        lp->perm_c = (long long*)lp->upload(P.perm_c);
+        lp->h_perm_r = P.perm_r; lp->h_perm_c = P.perm_c;
+        if (opt.keep_source_map) { lp->k_src = std::move(P.K.src); lp->k_lsrc = std::move(P.K.lsrc); lp->kt_src = std::move(P.KT.src); lp->kt_lsrc = std::move(P.KT.lsrc); }
+
+        Vecs& V = lp->V;
+        V.n = n; V.m = m;
+        for (int i = 0; i < 2; ++i) { V.x[i] = lp->dalloc<double>((size_t)n); V.y[i] = lp->dalloc<double>((size_t)m); }
+        V.xg = lp->dalloc<double2>((size_t)n);
+        V.xsum = lp->dalloc<double>((size_t)n); V.ysum = lp->dalloc<double>((size_t)m);
+        V.xr = lp->dalloc<double>((size_t)n); V.yr = lp->dalloc<double>((size_t)m);
+        lp->cs = lp->dalloc<double>((size_t)n); lp->ls = lp->dalloc<double>((size_t)n); lp->us = lp->dalloc<double>((size_t)n);
+        lp->qs = lp->dalloc<double>((size_t)m); lp->isG = lp->dalloc<unsigned char>((size_t)m);
+        lp->Dr = lp->dalloc<double>((size_t)m); lp->Dc = lp->dalloc<double>((size_t)n);
+        V.c = lp->cs; V.l = lp->ls; V.u = lp->us; V.q = lp->qs; V.isG = lp->isG; V.Dr = lp->Dr; V.Dc = lp->Dc;
+        V.gridA = lp->KT.grid; V.gridB = lp->K.grid; V.gridR = std::max(1, cdiv(n + m, kBlock));
+        V.partA = lp->dalloc<dd>((size_t)V.gridA);
+        V.partB = lp->dalloc<dd>((size_t)2 * V.gridB);
+        V.partD = lp->dalloc<dd>((size_t)8 * V.gridA);
+        V.partP = lp->dalloc<dd>((size_t)6 * V.gridB);
+        V.partR = lp->dalloc<dd>((size_t)2 * V.gridR);
+        lp->ctl = lp->dalloc<Ctrl>(1);
+        CK(cudaMemset(lp->ctl, 0, sizeof(Ctrl)));
+        CK(cudaHostAlloc((void**)&lp->h_status, sizeof(HostStatus), cudaHostAllocMapped));
+        CK(cudaHostAlloc((void**)&lp->h_stop, sizeof(int), cudaHostAllocMapped));
+        std::memset(lp->h_status, 0, sizeof(HostStatus)); *lp->h_stop = 0;
+        CK(cudaHostGetDevicePointer((void**)&lp->d_status, lp->h_status, 0));
+        CK(cudaHostGetDevicePointer((void**)&lp->d_stop, lp->h_stop, 0));
+
+        // original-order copies of the data vectors (temporary)
+        double *db = nullptr, *dc = nullptr, *dl = nullptr, *du = nullptr; char* dsense = nullptr;
+        auto tmp_up = [&](const void* h, size_t bytes) { void* p = nullptr; CK(cudaMalloc(&p, bytes ? bytes : 1)); if (bytes) CK(cudaMemcpy(p, h, bytes, cudaMemcpyHostToDevice)); return p; };
+        db = (double*)tmp_up(b, sizeof(double) * (size_t)m); dc = (double*)tmp_up(c, sizeof(double) * (size_t)n);
+        dl = (double*)tmp_up(l, sizeof(double) * (size_t)n); du = (double*)tmp_up(u, sizeof(double) * (size_t)n);
+        dsense = (char*)tmp_up(sense, (size_t)m);
+        dd* part = nullptr; double* scal = nullptr;
+        CK(cudaMalloc((void**)&part, sizeof(dd) * 1024)); CK(cudaMalloc((void**)&scal, sizeof(double)));
+
+        // unscaled norms for R9 (before anything is scaled)
+        lp->norm_b = std::sqrt(reduce_to_host(lp, db, m, 0, part, scal, st));
+        lp->norm_c = std::sqrt(reduce_to_host(lp, dc, n, 0, part, scal, st));
+
+        // A2, A3: preconditioning;  A4: scaled data and the initial scalars of R2
+        CK(cudaEventRecord(lp->ev_t0, st));
+        precondition(lp, st);
+        k_scale_problem<<<V.gridR, kBlock, 0, st>>>(n, m, db, dc, dl, du, dsense, lp->perm_c, lp->perm_r, lp->Dr, lp->Dc,
+                                                    lp->qs, lp->cs, lp->ls, lp->us, lp->isG);
+        CK(cudaGetLastError());
+        double kmax = reduce_to_host(lp, lp->K.val, lp->k_slots, 1, part, scal, st);
+        kmax = std::max(kmax, reduce_to_host(lp, lp->K.lval, lp->k_long_nnz, 1, part, scal, st));
+        const double ncs = std::sqrt(reduce_to_host(lp, lp->cs, n, 0, part, scal, st));
+        const double nqs = std::sqrt(reduce_to_host(lp, lp->qs, m, 0, part, scal, st));
+        CK(cudaEventRecord(lp->ev_t1, st));
+        CK(cudaStreamSynchronize(st));
+        float ms = 0.f; CK(cudaEventElapsedTime(&ms, lp->ev_t0, lp->ev_t1));
+        lp->precondition_seconds = ms * 1e-3;
+        lp->eta0 = kmax > 0.0 ? 1.0 / kmax : 1.0;
+        lp->omega0 = (ncs > 1e-10 && nqs > 1e-10) ? ncs / nqs : 1.0;
+        cudaFree(db); cudaFree(dc); cudaFree(dl); cudaFree(du); cudaFree(dsense); cudaFree(part); cudaFree(scal);
+        lp->create_seconds = now_s() - t_create;
+    } catch (const CudaFail& f) {
+        std::string msg = std::string(f.what) + ": " + cudaGetErrorString(f.e);
+        int code = (f.e == cudaErrorMemoryAllocation) ? UC_ERR_NOMEM : UC_ERR_CUDA;
+        destroy_impl(lp);
+        return fail(code, msg);
+    } catch (const std::bad_alloc&) {
+        destroy_impl(lp);
+        return fail(UC_ERR_NOMEM, "host allocation failed");
+    }
+    *out = lp;
+    return UC_OK;
+}
+
+void uc_lp_destroy(uc_lp* lp) { destroy_impl(lp); }
+
+int uc_lp_update_bounds(uc_lp* lp, const double* l_new, const double* u_new) {
+    if (!lp || (lp->n > 0 && (!l_new || !u_new))) return fail(UC_ERR_INVALID, "NULL argument");
+    for (int64_t j = 0; j < lp->n; ++j)
+        if (std::isnan(l_new[j]) || std::isnan(u_new[j]) || l_new[j] > u_new[j]) return fail(UC_ERR_INVALID, "bad bound");
+    int expected = 0;
+    if (!lp->busy.compare_exchange_strong(expected, 1)) return fail(UC_ERR_BUSY, "a solve is running on this handle");
+    int rc = UC_OK;
+    try {
+        DeviceGuard guard(lp->device);
+        double *dl = nullptr, *du = nullptr;
+        size_t bytes = sizeof(double) * (size_t)std::max<int64_t>(lp->n, 1);
+        CK(cudaMalloc((void**)&dl, bytes)); CK(cudaMalloc((void**)&du, bytes));
+        if (lp->n) { CK(cudaMemcpy(dl, l_new, sizeof(double) * (size_t)lp->n, cudaMemcpyHostToDevice)); CK(cudaMemcpy(du, u_new, sizeof(double) * (size_t)lp->n, cudaMemcpyHostToDevice)); }
+        k_scale_bounds<<<std::max(1, cdiv(lp->n, kBlock)), kBlock, 0, lp->own_stream>>>(lp->n, dl, du, lp->perm_c, lp->Dc, lp->ls, lp->us);
+        CK(cudaGetLastError());
+        CK(cudaStreamSynchronize(lp->own_stream));
+        cudaFree(dl); cudaFree(du);
+    } catch (const CudaFail& f) {
+        rc = fail(UC_ERR_CUDA, std::string(f.what) + ": " + cudaGetErrorString(f.e));
+    }
+    lp->busy.store(0);
+    return rc;
+}
+
+int uc_pdhg_cancel(uc_lp* lp) {
+    if (!lp) return fail(UC_ERR_INVALID, "handle is NULL");
+    lp->cancel_requested.store(1);
+    if (lp->h_stop) { *(volatile int*)lp->h_stop = UC_CANCELLED; }
+    return UC_OK;
+}
+
+static int solve_impl(uc_lp* lp, const uc_pdhg_params* pin, double* x_out, double* y_out, uc_pdhg_result* res, bool dev_io) {
+    if (!lp || !res) return fail(UC_ERR_INVALID, "handle or result is NULL");
+    uc_pdhg_params prm;
+    uc_pdhg_default_params(&prm);
+    if (pin) prm = *pin;
+    if (prm.check_every <= 0 || prm.iter_limit < 0 || prm.fixed_iterations < 0 || !(prm.eps_rel >= 0.0) || !(prm.eps_abs >= 0.0) ||
+        prm.attempt_trace_cap < 0 || prm.check_trace_cap < 0)
+        return fail(UC_ERR_INVALID, "bad uc_pdhg_params");
+    int expected = 0;
+    if (!lp->busy.compare_exchange_strong(expected, 1)) return fail(UC_ERR_BUSY, "a solve is already running on this handle");
+    std::memset(res, 0, sizeof *res);
+    const double t_wall = now_s();
+    int rc = UC_OK;
+    double *tx0 = nullptr, *ty0 = nullptr, *tx = nullptr, *ty = nullptr;
+    uc_attempt_record* d_att = nullptr; uc_check_record* d_chk = nullptr;
+    try {
+        DeviceGuard guard(lp->device);
+        cudaStream_t st = prm.stream ? (cudaStream_t)prm.stream : lp->own_stream;
+        const long long n = lp->n, m = lp->m;
+        const bool fixed = prm.fixed_iterations > 0;
+        const long long limit = fixed ? prm.fixed_iterations : prm.iter_limit;
+        const int ce = prm.check_every;
+
+        // a cancel that arrived before the solve started is honoured here (PAPER.md l.80-85 race)
+        if (lp->cancel_requested.exchange(0)) {
+            *(volatile int*)lp->h_stop = 0;
+            res->status = UC_CANCELLED;
+            res->solve_seconds = now_s() - t_wall;
+            lp->busy.store(0);
+            return UC_OK;
+        }
+        *(volatile int*)lp->h_stop = 0;
+        if (lp->cancel_requested.load()) *(volatile int*)lp->h_stop = UC_CANCELLED;   // cancel raced with the reset
+        std::memset(lp->h_status, 0, sizeof(HostStatus));
+
+        // warm start
+        const double *dx0 = nullptr, *dy0 = nullptr;
+        if (prm.x0) {
+            if (dev_io) dx0 = prm.x0;
+            else { CK(cudaMalloc((void**)&tx0, sizeof(double) * (size_t)std::max<long long>(n, 1))); CK(cudaMemcpyAsync(tx0, prm.x0, sizeof(double) * (size_t)n, cudaMemcpyHostToDevice, st)); dx0 = tx0; }
+        }
+        if (prm.y0) {
+            if (dev_io) dy0 = prm.y0;
+            else { CK(cudaMalloc((void**)&ty0, sizeof(double) * (size_t)std::max<long long>(m, 1))); CK(cudaMemcpyAsync(ty0, prm.y0, sizeof(double) * (size_t)m, cudaMemcpyHostToDevice, st)); dy0 = ty0; }
+        }
+        if (prm.attempt_trace && prm.attempt_trace_cap > 0) CK(cudaMalloc((void**)&d_att, sizeof(uc_attempt_record) * (size_t)prm.attempt_trace_cap));
+        if (prm.check_trace && prm.check_trace_cap > 0) CK(cudaMalloc((void**)&d_chk, sizeof(uc_check_record) * (size_t)prm.check_trace_cap));
+
+        ensure_powtab(lp, limit);
+        // R2: control block
+        Ctrl h{};
+        h.eta = lp->eta0; h.omega = lp->omega0; h.eta_prev = 0.0; h.w = 0.0; h.mu_prev = INFINITY;
+        h.limit = limit; h.fixed = fixed ? 1 : 0; h.status = UC_ITERATION_LIMIT;
+        h.eps_abs = prm.eps_abs; h.eps_rel = prm.eps_rel; h.beta_s = prm.beta_sufficient; h.beta_n = prm.beta_necessary;
+        h.beta_a = prm.beta_artificial; h.smoothing = prm.weight_smoothing; h.norm_q = lp->norm_b; h.norm_c = lp->norm_c;
+        h.att = d_att; h.att_cap = d_att ? prm.attempt_trace_cap : 0; h.chk = d_chk; h.chk_cap = d_chk ? prm.check_trace_cap : 0;
+        h.host_stop = lp->d_stop; h.host_status = lp->d_status; h.powtab = lp->powtab;
+        CK(cudaMemcpyAsync(lp->ctl, &h, sizeof(Ctrl), cudaMemcpyHostToDevice, st));
+        int64_t launches = 0;
+        k_init_point<<<lp->V.gridR, kBlock, 0, st>>>(lp->V, dx0, dy0, lp->perm_c, lp->perm_r);
+        launch_kkt(lp, st, kModeInit);                     // KKT components of the restart point z^0
+        launches += 4;
+        CK(cudaGetLastError());
+        CK(cudaStreamSynchronize(st));                     // the pageable Ctrl copy and tx0/ty0 are consumed
+        build_graph(lp, ce);
+
+        // ---- the loop: one graph launch = `ce` attempts + one check; two launches kept in flight
+        CK(cudaEventRecord(lp->ev_t0, st));
+        const long long nblocks = limit / ce, rem = limit % ce;
+        const int depth = 2;
+        bool done = false;
+        long long b = 0;
+        for (; b < nblocks && !done; ++b) {
+            CK(cudaGraphLaunch(lp->exec, st));
+            launches += lp->graph_nodes;
+            CK(cudaEventRecord(lp->ev[b % depth], st));
+            if (b >= depth - 1) {
+                CK(cudaEventSynchronize(lp->ev[(b - depth + 1) % depth]));
+                if (((volatile HostStatus*)lp->h_status)->done) done = true;
+                if (!done && now_s() - t_wall > prm.time_limit_s && *(volatile int*)lp->h_stop == 0) *(volatile int*)lp->h_stop = UC_TIME_LIMIT;
+            }
+        }
+        CK(cudaStreamSynchronize(st));
+        done = ((volatile HostStatus*)lp->h_status)->done != 0;
+        if (!done && rem > 0) {
+            for (long long r = 0; r < rem; ++r) launch_attempt(lp, st);
+            launches += 2 * rem;
+            if (!fixed) { launch_check(lp, st); launches += kCheckLaunches; }
+            CK(cudaStreamSynchronize(st));
+            done = ((volatile HostStatus*)lp->h_status)->done != 0;
+        }
+        CK(cudaEventRecord(lp->ev_t1, st));
+        if (!done) {                                       // fixed-iteration end (R14) or iter_limit = 0: report only
+            launch_kkt(lp, st, kModeReport);
+            launches += 3;
+        }
+        // ---- A14: unscale, un-permute, hand back
+        double* ox = x_out; double* oy = y_out;
+        if (!dev_io) {
+            if (x_out) { CK(cudaMalloc((void**)&tx, sizeof(double) * (size_t)std::max<long long>(n, 1))); ox = tx; }
+            if (y_out) { CK(cudaMalloc((void**)&ty, sizeof(double) * (size_t)std::max<long long>(m, 1))); oy = ty; }
+        }
+        if (ox || oy) { k_output<<<lp->V.gridR, kBlock, 0, st>>>(lp->V, lp->ctl, ox, oy, lp->perm_c, lp->perm_r); launches += 1; }
+        CK(cudaGetLastError());
+        if (!dev_io) {
+            if (x_out && n) CK(cudaMemcpyAsync(x_out, tx, sizeof(double) * (size_t)n, cudaMemcpyDeviceToHost, st));
+            if (y_out && m) CK(cudaMemcpyAsync(y_out, ty, sizeof(double) * (size_t)m, cudaMemcpyDeviceToHost, st));
+        }
+        Ctrl hc;
+        CK(cudaMemcpyAsync(&hc, lp->ctl, sizeof(Ctrl), cudaMemcpyDeviceToHost, st));
+        if (d_att) { long long cnt = std::min<long long>(prm.attempt_trace_cap, limit); if (cnt > 0) CK(cudaMemcpyAsync(prm.attempt_trace, d_att, sizeof(uc_attempt_record) * (size_t)cnt, cudaMemcpyDeviceToHost, st)); }
+        if (d_chk) CK(cudaMemcpyAsync(prm.check_trace, d_chk, sizeof(uc_check_record) * (size_t)prm.check_trace_cap, cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        float ms = 0.f; CK(cudaEventElapsedTime(&ms, lp->ev_t0, lp->ev_t1));
+
+        const HostStatus hs = *lp->h_status;
+        res->status = hc.status; res->returned_average = hc.ret_avg;
+        res->iterations = hc.k; res->accepted = hc.accepted; res->restarts = hc.restarts;
+        res->rel_kkt = hs.rel_kkt; res->rel_primal_res = hs.rel_rp; res->rel_dual_res = hs.rel_rd; res->rel_gap = hs.rel_gap;
+        res->primal_obj = hs.pobj; res->dual_obj = hs.dobj; res->eta = hc.eta; res->omega = hc.omega;
+        res->loop_seconds = ms * 1e-3;
+        res->attempt_records = hc.k; res->check_records = hc.nchk;
+        res->kernel_launches = launches;
+        if (hc.status == UC_CANCELLED) lp->cancel_requested.store(0);
+        *(volatile int*)lp->h_stop = 0;
+        if (lp->cancel_requested.load()) *(volatile int*)lp->h_stop = UC_CANCELLED;   // arrived after the last check: stays sticky
+    } catch (const CudaFail& f) {
+        rc = fail((f.e == cudaErrorMemoryAllocation) ? UC_ERR_NOMEM : UC_ERR_CUDA, std::string(f.what) + ": " + cudaGetErrorString(f.e));
+    }
+    if (tx0) cudaFree(tx0);
+    if (ty0) cudaFree(ty0);
+    if (tx) cudaFree(tx);
+    if (ty) cudaFree(ty);
+    if (d_att) cudaFree(d_att);
+    if (d_chk) cudaFree(d_chk);
+    res->solve_seconds = now_s() - t_wall;
+    lp->busy.store(0);
+    return rc;
+}
+
+int uc_pdhg_solve(uc_lp* lp, const uc_pdhg_params* p, double* x_out, double* y_out, uc_pdhg_result* res) {
+    return solve_impl(lp, p, x_out, y_out, res, false);
+}
+int uc_pdhg_solve_device(uc_lp* lp, const uc_pdhg_params* p, double* x_out, double* y_out, uc_pdhg_result* res) {
+    return solve_impl(lp, p, x_out, y_out, res, true);
+}
+
+int uc_lp_get_info(const uc_lp* lp, uc_lp_info* info) {
+    if (!lp || !info) return fail(UC_ERR_INVALID, "NULL argument");
+    std::memset(info, 0, sizeof *info);
+    info->m = lp->m; info->n = lp->n; info->nnz = lp->nnz;
+    info->k_sell_slots = lp->k_slots; info->kt_sell_slots = lp->kt_slots;
+    info->k_long_rows = lp->K.nlong; info->kt_long_rows = lp->KT.nlong;
+    info->k_long_nnz = lp->k_long_nnz; info->kt_long_nnz = lp->kt_long_nnz;
+    info->device_bytes = (int64_t)lp->device_bytes;
+    info->precondition_seconds = lp->precondition_seconds; info->create_seconds = lp->create_seconds;
+    info->eta0 = lp->eta0; info->omega0 = lp->omega0; info->norm_b = lp->norm_b; info->norm_c = lp->norm_c;
+    info->bytes_per_attempt = bytes_per_attempt(lp);
+    return UC_OK;
+}
+
+int uc_lp_get_scaling(uc_lp* lp, double* Dr_out, double* Dc_out) {
+    if (!lp) return fail(UC_ERR_INVALID, "handle is NULL");
+    try {
+        DeviceGuard guard(lp->device);
+        std::vector<double> t;
+        if (Dr_out) {
+            t.resize((size_t)lp->m);
+            if (lp->m) CK(cudaMemcpy(t.data(), lp->Dr, sizeof(double) * (size_t)lp->m, cudaMemcpyDeviceToHost));
+            for (int64_t k = 0; k < lp->m; ++k) Dr_out[lp->h_perm_r[(size_t)k]] = t[(size_t)k];
+        }
+        if (Dc_out) {
+            t.resize((size_t)lp->n);
+            if (lp->n) CK(cudaMemcpy(t.data(), lp->Dc, sizeof(double) * (size_t)lp->n, cudaMemcpyDeviceToHost));
+            for (int64_t k = 0; k < lp->n; ++k) Dc_out[lp->h_perm_c[(size_t)k]] = t[(size_t)k];
+        }
+    } catch (const CudaFail& f) {
+        return fail(UC_ERR_CUDA, std::string(f.what) + ": " + cudaGetErrorString(f.e));
+    }
+    return UC_OK;
+}
+
+int uc_lp_get_scaled_values(uc_lp* lp, int32_t from_transpose, double* val_out) {
+    if (!lp || (lp->nnz > 0 && !val_out)) return fail(UC_ERR_INVALID, "NULL argument");
+    if (!lp->opt.keep_source_map) return fail(UC_ERR_INVALID, "handle was created without keep_source_map");
+    try {
+        DeviceGuard guard(lp->device);
+        const Sell& S = from_transpose ? lp->KT : lp->K;
+        const std::vector<int64_t>& src = from_transpose ? lp->kt_src : lp->k_src;
+        const std::vector<int64_t>& lsrc = from_transpose ? lp->kt_lsrc : lp->k_lsrc;
+        std::vector<double> t(src.size());
+        if (!t.empty()) CK(cudaMemcpy(t.data(), S.val, sizeof(double) * t.size(), cudaMemcpyDeviceToHost));
+        for (size_t k = 0; k < src.size(); ++k) if (src[k] >= 0) val_out[src[k]] = t[k];
+        t.resize(lsrc.size());
+        if (!t.empty()) CK(cudaMemcpy(t.data(), S.lval, sizeof(double) * t.size(), cudaMemcpyDeviceToHost));
+        for (size_t k = 0; k < lsrc.size(); ++k) val_out[lsrc[k]] = t[k];
+    } catch (const CudaFail& f) {
+        return fail(UC_ERR_CUDA, std::string(f.what) + ": " + cudaGetErrorString(f.e));
+    }
+    return UC_OK;
+}
+
+int uc_lp_spmv(uc_lp* lp, int32_t transpose, const double* v, double* out) {
+    if (!lp || !v || !out) return fail(UC_ERR_INVALID, "NULL argument");
+    int expected = 0;
+    if (!lp->busy.compare_exchange_strong(expected, 1)) return fail(UC_ERR_BUSY, "a solve is running on this handle");
+    int rc = UC_OK;
+    double *din = nullptr, *dperm = nullptr, *dres = nullptr, *dout = nullptr;
+    try {
+        DeviceGuard guard(lp->device);
+        const long long nin = transpose ? lp->m : lp->n, nout = transpose ? lp->n : lp->m;
+        const long long* pin = transpose ? lp->perm_r : lp->perm_c;
+        const long long* pout = transpose ? lp->perm_c : lp->perm_r;
+        const Sell& S = transpose ? lp->KT : lp->K;
+        cudaStream_t st = lp->own_stream;
+        CK(cudaMalloc((void**)&din, sizeof(double) * (size_t)std::max<long long>(nin, 1)));
+        CK(cudaMalloc((void**)&dperm, sizeof(double) * (size_t)std::max<long long>(nin, 1)));
+        CK(cudaMalloc((void**)&dres, sizeof(double) * (size_t)std::max<long long>(nout, 1)));
+        CK(cudaMalloc((void**)&dout, sizeof(double) * (size_t)std::max<long long>(nout, 1)));
+        if (nin) CK(cudaMemcpyAsync(din, v, sizeof(double) * (size_t)nin, cudaMemcpyHostToDevice, st));
+        k_gather<<<std::max(1, cdiv(nin, 256)), 256, 0, st>>>(din, pin, nin, dperm);
+        k_spmv<<<S.grid, kBlock, 0, st>>>(S, dperm, dres);
+        k_scatter<<<std::max(1, cdiv(nout, 256)), 256, 0, st>>>(dres, pout, nout, dout);
+        CK(cudaGetLastError());
+        if (nout) CK(cudaMemcpyAsync(out, dout, sizeof(double) * (size_t)nout, cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+    } catch (const CudaFail& f) {
+        rc = fail(UC_ERR_CUDA, std::string(f.what) + ": " + cudaGetErrorString(f.e));
+    }
+    if (din) cudaFree(din);
+    if (dperm) cudaFree(dperm);
+    if (dres) cudaFree(dres);
+    if (dout) cudaFree(dout);
+    lp->busy.store(0);
+    return rc;
+}
+
+}  // extern "C"
