@@ -153,6 +153,12 @@ int uc_pdhg_solve_device(uc_lp* lp, const uc_pdhg_params* params, double* x_out_
    is not lost (the race of Algorithm 1). */
 int uc_pdhg_cancel(uc_lp* lp);
 
+/* Measurement hook: from the initial point, run `attempts` attempts as plain stream
+   launches with a CUDA event between the two kernels and return the average device time, in ms, of
+   the primal kernel (K' pass, A5+A6) and of the dual kernel (K pass, A7..A9).  stream: cudaStream_t or
+   NULL.  The handle's iterate state is overwritten. */
+int uc_pdhg_time_kernels(uc_lp* lp, void* stream, int32_t attempts, double* primal_ms, double* dual_ms);
+
 /* ------------------------------------------------------------------------------- introspection */
 typedef struct {
     int64_t m, n, nnz;

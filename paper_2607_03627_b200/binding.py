@@ -60,7 +60,7 @@ CHECK_DTYPE = np.dtype([("k", "i8"), ("restart_kind", "i4"), ("candidate", "i4")
                         ("mu_c", "f8"), ("mu_r", "f8"), ("relkkt_cur", "f8"), ("relkkt_avg", "f8")])
 
 EXPORTS = ["uc_lp_default_options", "uc_lp_create", "uc_lp_update_bounds", "uc_lp_destroy",
-           "uc_pdhg_default_params", "uc_pdhg_solve", "uc_pdhg_solve_device", "uc_pdhg_cancel",
+           "uc_pdhg_default_params", "uc_pdhg_solve", "uc_pdhg_solve_device", "uc_pdhg_cancel", "uc_pdhg_time_kernels",
            "uc_lp_get_info", "uc_lp_get_scaling", "uc_lp_get_scaled_values", "uc_lp_spmv", "uc_last_error",
            "uc_host_log_rounded", "uc_host_exp_rounded"]
 
@@ -95,6 +95,7 @@ def load_library(build_if_missing: bool = True):
     lib.uc_lp_update_bounds.argtypes = [C.c_void_p] * 3
     lib.uc_pdhg_solve.argtypes = [C.c_void_p] * 5
     lib.uc_pdhg_solve_device.argtypes = [C.c_void_p] * 5
+    lib.uc_pdhg_time_kernels.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
     lib.uc_lp_get_info.argtypes = [C.c_void_p] * 2
     lib.uc_lp_get_scaling.argtypes = [C.c_void_p] * 3
     lib.uc_lp_get_scaled_values.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
@@ -200,6 +201,15 @@ class UcLp:
         _check(self.lib.uc_lp_update_bounds(self._h, lp_, up_))
 
     update_bounds = uc_lp_update_bounds
+
+    def uc_pdhg_time_kernels(self, attempts=64, stream=None):
+        """(primal_ms, dual_ms): average device time of the two kernels of an attempt (CUDA events)."""
+        a, b = C.c_double(0.0), C.c_double(0.0)
+        _check(self.lib.uc_pdhg_time_kernels(self._h, C.c_void_p(int(stream)) if stream else None, int(attempts),
+                                             C.cast(C.byref(a), C.c_void_p), C.cast(C.byref(b), C.c_void_p)))
+        return a.value, b.value
+
+    time_kernels = uc_pdhg_time_kernels
 
     def info(self) -> Info:
         i = Info()

@@ -182,6 +182,25 @@ void launch_check(uc_lp* lp, cudaStream_t st) {
 }
 constexpr int kCheckLaunches = 6;
 
+// R2: control block, initial point, KKT components of the restart point z^0 (4 launches); synchronises `st`.
+void start_run(uc_lp* lp, const uc_pdhg_params& prm, cudaStream_t st, long long limit, bool fixed,
+               const double* dx0, const double* dy0, uc_attempt_record* d_att, uc_check_record* d_chk) {
+    ensure_powtab(lp, limit);
+    Ctrl h{};
+    h.eta = lp->eta0; h.omega = lp->omega0; h.eta_prev = 0.0; h.w = 0.0; h.mu_prev = INFINITY;
+    h.limit = limit; h.fixed = fixed ? 1 : 0; h.status = UC_ITERATION_LIMIT;
+    h.eps_abs = prm.eps_abs; h.eps_rel = prm.eps_rel; h.beta_s = prm.beta_sufficient; h.beta_n = prm.beta_necessary;
+    h.beta_a = prm.beta_artificial; h.smoothing = prm.weight_smoothing; h.norm_q = lp->norm_b; h.norm_c = lp->norm_c;
+    h.att = d_att; h.att_cap = d_att ? prm.attempt_trace_cap : 0; h.chk = d_chk; h.chk_cap = d_chk ? prm.check_trace_cap : 0;
+    h.host_stop = lp->d_stop; h.host_status = lp->d_status; h.powtab = lp->powtab;
+    CK(cudaMemcpyAsync(lp->ctl, &h, sizeof(Ctrl), cudaMemcpyHostToDevice, st));
+    k_init_point<<<lp->V.gridR, kBlock, 0, st>>>(lp->V, dx0, dy0, lp->perm_c, lp->perm_r);
+    launch_kkt(lp, st, kModeInit);
+    CK(cudaGetLastError());
+    CK(cudaStreamSynchronize(st));                     // the pageable Ctrl copy and any staged warm start are consumed
+}
+
+
 // capture `ce` attempts + one check into an executable graph (A15)
 void build_graph(uc_lp* lp, int ce) {
     if (lp->exec && lp->graph_ce == ce) return;
@@ -437,22 +456,9 @@ static int solve_impl(uc_lp* lp, const uc_pdhg_params* pin, double* x_out, doubl
         if (prm.attempt_trace && prm.attempt_trace_cap > 0) CK(cudaMalloc((void**)&d_att, sizeof(uc_attempt_record) * (size_t)prm.attempt_trace_cap));
         if (prm.check_trace && prm.check_trace_cap > 0) CK(cudaMalloc((void**)&d_chk, sizeof(uc_check_record) * (size_t)prm.check_trace_cap));
 
-        ensure_powtab(lp, limit);
-        // R2: control block
-        Ctrl h{};
-        h.eta = lp->eta0; h.omega = lp->omega0; h.eta_prev = 0.0; h.w = 0.0; h.mu_prev = INFINITY;
-        h.limit = limit; h.fixed = fixed ? 1 : 0; h.status = UC_ITERATION_LIMIT;
-        h.eps_abs = prm.eps_abs; h.eps_rel = prm.eps_rel; h.beta_s = prm.beta_sufficient; h.beta_n = prm.beta_necessary;
-        h.beta_a = prm.beta_artificial; h.smoothing = prm.weight_smoothing; h.norm_q = lp->norm_b; h.norm_c = lp->norm_c;
-        h.att = d_att; h.att_cap = d_att ? prm.attempt_trace_cap : 0; h.chk = d_chk; h.chk_cap = d_chk ? prm.check_trace_cap : 0;
-        h.host_stop = lp->d_stop; h.host_status = lp->d_status; h.powtab = lp->powtab;
-        CK(cudaMemcpyAsync(lp->ctl, &h, sizeof(Ctrl), cudaMemcpyHostToDevice, st));
         int64_t launches = 0;
-        k_init_point<<<lp->V.gridR, kBlock, 0, st>>>(lp->V, dx0, dy0, lp->perm_c, lp->perm_r);
-        launch_kkt(lp, st, kModeInit);                     // KKT components of the restart point z^0
+        start_run(lp, prm, st, limit, fixed, dx0, dy0, d_att, d_chk);
         launches += 4;
-        CK(cudaGetLastError());
-        CK(cudaStreamSynchronize(st));                     // the pageable Ctrl copy and tx0/ty0 are consumed
         build_graph(lp, ce);
 
         // ---- the loop: one graph launch = `ce` attempts + one check; two launches kept in flight
@@ -534,6 +540,44 @@ int uc_pdhg_solve(uc_lp* lp, const uc_pdhg_params* p, double* x_out, double* y_o
 }
 int uc_pdhg_solve_device(uc_lp* lp, const uc_pdhg_params* p, double* x_out, double* y_out, uc_pdhg_result* res) {
     return solve_impl(lp, p, x_out, y_out, res, true);
+}
+
+int uc_pdhg_time_kernels(uc_lp* lp, void* stream, int32_t attempts, double* primal_ms, double* dual_ms) {
+    if (!lp || attempts <= 0 || !primal_ms || !dual_ms) return fail(UC_ERR_INVALID, "bad argument");
+    int expected = 0;
+    if (!lp->busy.compare_exchange_strong(expected, 1)) return fail(UC_ERR_BUSY, "a solve is running on this handle");
+    int rc = UC_OK;
+    std::vector<cudaEvent_t> ev;
+    try {
+        DeviceGuard guard(lp->device);
+        cudaStream_t st = stream ? (cudaStream_t)stream : lp->own_stream;
+        uc_pdhg_params prm; uc_pdhg_default_params(&prm);
+        const int warm = 8;
+        start_run(lp, prm, st, (long long)attempts + warm, true, nullptr, nullptr, nullptr, nullptr);
+        for (int i = 0; i < warm; ++i) launch_attempt(lp, st);
+        ev.resize((size_t)2 * attempts + 1);
+        for (auto& e : ev) CK(cudaEventCreate(&e));
+        CK(cudaEventRecord(ev[0], st));
+        for (int i = 0; i < attempts; ++i) {
+            k_primal<<<lp->KT.grid, kBlock, 0, st>>>(lp->KT, lp->V, lp->ctl);
+            CK(cudaEventRecord(ev[(size_t)2 * i + 1], st));
+            k_dual<<<lp->K.grid, kBlock, 0, st>>>(lp->K, lp->V, lp->ctl);
+            CK(cudaEventRecord(ev[(size_t)2 * i + 2], st));
+        }
+        CK(cudaStreamSynchronize(st));
+        double a = 0.0, b = 0.0;
+        for (int i = 0; i < attempts; ++i) {
+            float ms = 0.f;
+            CK(cudaEventElapsedTime(&ms, ev[(size_t)2 * i], ev[(size_t)2 * i + 1])); a += ms;
+            CK(cudaEventElapsedTime(&ms, ev[(size_t)2 * i + 1], ev[(size_t)2 * i + 2])); b += ms;
+        }
+        *primal_ms = a / attempts; *dual_ms = b / attempts;
+    } catch (const CudaFail& f) {
+        rc = fail(UC_ERR_CUDA, std::string(f.what) + ": " + cudaGetErrorString(f.e));
+    }
+    for (auto& e : ev) if (e) cudaEventDestroy(e);
+    lp->busy.store(0);
+    return rc;
 }
 
 int uc_lp_get_info(const uc_lp* lp, uc_lp_info* info) {

@@ -1,0 +1,105 @@
+"""ABI behaviour on a GPU (-m gpu): cancel ("Terminate the other solver"), busy handle,
+time limit, device-pointer entry point, the paper's stopping knobs."""
+import threading
+import time
+
+import numpy as np
+import pytest
+
+import oracle
+import paper_2607_03627_b200 as P
+from workloads import uc_config
+
+from helpers import rel_l2
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def lp1():
+    return uc_config(1)
+
+
+def test_cancel_before_solve_is_not_lost(lp1):
+    with P.UcLp(lp1) as h:
+        h.cancel()
+        s = h.solve()
+        assert s.status == P.CANCELLED and s.iterations == 0
+        s = h.solve(fixed_iterations=64)                  # flag was consumed: the handle is reusable
+        assert s.status == P.ITERATION_LIMIT and s.iterations == 64
+
+
+def test_cancel_from_another_thread_stops_within_a_few_checks(lp1):
+    with P.UcLp(lp1) as h:
+        ref = h.solve(fixed_iterations=64 * 40)            # measure the pace: seconds per check block
+        per_block = ref.loop_seconds / 40
+        out = {}
+
+        def run():
+            out["s"] = h.solve(iter_limit=10_000_000, eps_rel=0.0, eps_abs=0.0)
+
+        t = threading.Thread(target=run)
+        t.start()
+        time.sleep(0.2)
+        with pytest.raises(P.UcError) as e:                # a second solve on the same handle is refused
+            h.solve(fixed_iterations=1)
+        assert e.value.code == -4
+        t0 = time.time()
+        h.cancel()
+        t.join(timeout=30)
+        latency = time.time() - t0
+        assert not t.is_alive()
+        s = out["s"]
+        assert s.status == P.CANCELLED and s.iterations % 64 == 0 and s.iterations > 0
+        assert latency < max(0.25, 20 * per_block)         # far below the 0.5 s poll of Algorithm 1
+        again = h.solve(fixed_iterations=64)               # handle reusable, flag cleared
+        assert again.status == P.ITERATION_LIMIT
+
+
+def test_time_limit(lp1):
+    with P.UcLp(lp1) as h:
+        s = h.solve(iter_limit=50_000_000, eps_rel=0.0, eps_abs=0.0, time_limit_s=0.3)
+        assert s.status == P.TIME_LIMIT and 0.25 < s.solve_seconds < 3.0
+
+
+def test_paper_stopping_knobs(lp1):
+    """iteration limit 100,000, absolute feasibility tolerance 1e-5, convergence tolerance 1e-4."""
+    p = P.default_params()
+    assert p.iter_limit == 100000 and p.eps_rel == 1e-4 and p.check_every == 64
+    lp = uc_config(0)
+    with P.UcLp(lp) as h:
+        loose = h.solve()
+        tight = h.solve(eps_abs=1e-5)
+    so = oracle.solve(lp, eps_abs=1e-5)
+    assert tight.status == P.OPTIMAL and tight.iterations >= loose.iterations
+    assert tight.iterations == so.iterations
+
+
+def test_device_pointer_entry_point_with_torch_memory_and_stream(lp1):
+    import torch
+    dev = torch.device("cuda:0")
+    x = torch.empty(lp1.n, dtype=torch.float64, device=dev)
+    y = torch.empty(lp1.m, dtype=torch.float64, device=dev)
+    stream = torch.cuda.Stream()
+    with P.UcLp(lp1) as h:
+        host = h.solve(fixed_iterations=128)
+        with torch.cuda.stream(stream):
+            s = h.solve_device(x, y, fixed_iterations=128, stream=stream.cuda_stream)
+        stream.synchronize()
+        np.testing.assert_array_equal(x.cpu().numpy(), host.x)
+        np.testing.assert_array_equal(y.cpu().numpy(), host.y)
+        # warm start from device tensors: continue 72 more attempts is NOT the same trajectory (state resets), but it must run
+        s2 = h.solve_device(x, y, x0=x.clone(), y0=y.clone(), fixed_iterations=8, stream=stream.cuda_stream)
+        assert s2.iterations == 8 and s.kernel_launches > 2 * 128
+
+
+def test_info_and_launch_count(lp1):
+    with P.UcLp(lp1) as h:
+        i = h.info()
+        assert (i.m, i.n, i.nnz) == (lp1.m, lp1.n, lp1.nnz)
+        assert i.k_sell_slots + i.k_long_nnz >= lp1.nnz and i.kt_sell_slots + i.kt_long_nnz >= lp1.nnz
+        assert i.k_long_rows == lp1.meta["T"]                      # the T reserve rows (G = 90 entries) form the long tail
+        assert (i.k_sell_slots + i.k_long_nnz) / lp1.nnz < 1.03    # sliced-ELL padding stays below 3 %
+        assert i.bytes_per_attempt > 24 * lp1.nnz
+        s = h.solve(fixed_iterations=128)
+        assert s.kernel_launches >= 2 * 128 + 2 * 6

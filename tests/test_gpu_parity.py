@@ -1,0 +1,293 @@
+"""GPU parity tests (-m gpu): the CUDA path, called through the C ABI (ctypes binding), against the CPU
+oracle on the same seeded inputs.  Bars (BASELINE.json north_star): after a fixed 200 attempts the
+iterates agree within 1e-10 relative L2 (x and y separately) with identical accept / restart traces;
+at convergence (relative KKT <= 1e-4) objectives agree within 1e-5 relative.  Integer / index work
+(layout round trip, K' == CSC(K)) is compared bit-exactly."""
+import json
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+import paper_2607_03627_b200 as P
+from workloads import tiny, uc_config, random_lp, fix_commitment
+from workloads.lp import LP, from_dense
+
+from helpers import rel_l2, highs, GOLDEN
+
+pytestmark = pytest.mark.gpu
+
+TOL_ITER = 1e-10     # north_star: iterates after 200 fixed attempts, relative L2
+TOL_OBJ = 1e-5       # north_star: objectives at convergence, relative
+
+
+def ragged_lp(seed=5, n=3000, m=2500):
+    """Random LP with empty rows, empty columns, a few rows far longer than the sliced-ELL threshold
+    and a ragged tail (sizes not multiples of 32)."""
+    rng = np.random.default_rng(seed)
+    n, m = n + 7, m + 13
+    lens = rng.integers(0, 9, m)
+    lens[rng.integers(0, m, 5)] = rng.integers(40, 400, 5)          # long tail rows
+    lens[:3] = 0
+    rows, cols = [], []
+    for i, k in enumerate(lens):
+        c = rng.choice(n - 11, size=int(k), replace=False)           # last 11 columns stay empty
+        rows += [i] * int(k); cols += c.tolist()
+    vals = rng.standard_normal(len(rows)) * rng.choice([0.01, 1.0, 50.0], len(rows))
+    l = -rng.uniform(0, 5, n); u = rng.uniform(0, 5, n)
+    l[rng.integers(0, n, 40)] = -np.inf; u[rng.integers(0, n, 40)] = np.inf
+    x0 = np.clip(rng.standard_normal(n), np.maximum(l, -3), np.minimum(u, 3))
+    from workloads.lp import from_coo
+    sense = np.where(rng.uniform(size=m) < 0.4, ord("E"), ord("G")).astype(np.uint8)
+    lp = from_coo(m, n, rows, cols, vals, sense, np.zeros(m), rng.standard_normal(n), l, u, name="ragged")
+    lp.b = lp.to_scipy() @ x0 - np.where(sense == ord("G"), rng.uniform(0, 1, m), 0.0)
+    return lp
+
+
+CASES = {
+    "one_by_one": tiny.one_by_one,
+    "two_var": tiny.two_var,
+    "box_only": lambda: tiny.box_only(),
+    "box_rows": lambda: tiny.box_only(with_rows=3),
+    "free_var": tiny.free_var_lp,
+    "small_random": lambda: tiny.small_random(6, 4, 1),
+    "dispatch": lambda: tiny.economic_dispatch()[0],
+    "ragged": ragged_lp,
+    "uc0": lambda: uc_config(0),
+    "uc1": lambda: uc_config(1),
+    "random_2e4": lambda: random_lp(20_000, 21),
+}
+_lp_cache = {}
+
+
+def get_lp(name):
+    if name not in _lp_cache:
+        _lp_cache[name] = CASES[name]()
+    return _lp_cache[name]
+
+
+def assert_trajectory_parity(lp, F=200, **opts):
+    so = oracle.solve(lp, fixed_iterations=F, trace_attempts=F, trace_checks=64)
+    with P.UcLp(lp, **opts) as h:
+        sg = h.solve(fixed_iterations=F, trace_attempts=F, trace_checks=64)
+    assert sg.status == P.ITERATION_LIMIT and sg.iterations == F == so.iterations
+    np.testing.assert_array_equal(sg.attempts["accepted"], so.attempts["accepted"])
+    np.testing.assert_array_equal(sg.checks["k"], so.checks["k"])
+    np.testing.assert_array_equal(sg.checks["restart_kind"], so.checks["restart_kind"])
+    np.testing.assert_array_equal(sg.checks["candidate"], so.checks["candidate"])
+    assert rel_l2(sg.x, so.x) <= TOL_ITER, "x after %d attempts" % F
+    if lp.m:
+        assert rel_l2(sg.y, so.y) <= TOL_ITER, "y after %d attempts" % F
+    np.testing.assert_allclose(sg.attempts["eta_used"], so.attempts["eta_used"], rtol=1e-9)
+    assert sg.accepted == so.accepted and sg.restarts == so.restarts
+    assert sg.omega == pytest.approx(so.omega, rel=1e-9) and sg.eta == pytest.approx(so.eta, rel=1e-9)
+    assert sg.primal_obj == pytest.approx(so.primal_obj, rel=1e-9, abs=1e-9)
+    assert sg.rel_kkt == pytest.approx(so.rel_kkt, rel=1e-6, abs=1e-12)
+    return sg, so
+
+
+# ------------------------------------------------------------------ R1: preconditioner + layouts
+@pytest.mark.parametrize("name", ["two_var", "small_random", "ragged", "uc0", "uc1", "random_2e4"])
+def test_preconditioner_matches_oracle(name):
+    lp = get_lp(name)
+    vs, Dr, Dc = oracle.precondition(lp)
+    with P.UcLp(lp, keep_source_map=1) as h:
+        gDr, gDc = h.scaling()
+        v_k, v_kt = h.scaled_values(False), h.scaled_values(True)
+    np.testing.assert_allclose(gDr, Dr, rtol=1e-14)
+    np.testing.assert_allclose(gDc, Dc, rtol=1e-14)
+    np.testing.assert_allclose(v_k, vs, rtol=1e-14)
+    np.testing.assert_array_equal(v_k, v_kt)          # K' is the CSC of K, bit for bit, after 11 scaling passes
+
+
+@pytest.mark.parametrize("alpha,ruiz", [(0.0, 10), (1.0, 0), (0.0, 0)])
+def test_preconditioner_options(alpha, ruiz):
+    lp = get_lp("uc0")
+    vs, Dr, Dc = oracle.precondition(lp, ruiz_iters=ruiz, pc_alpha=alpha)
+    with P.UcLp(lp, keep_source_map=1, ruiz_iters=ruiz, pc_alpha=alpha) as h:
+        gDr, gDc = h.scaling()
+        np.testing.assert_allclose(h.scaled_values(False), vs, rtol=1e-14)
+    np.testing.assert_allclose(gDr, Dr, rtol=1e-14)
+    np.testing.assert_allclose(gDc, Dc, rtol=1e-14)
+
+
+@pytest.mark.parametrize("name", ["small_random", "ragged", "uc1"])
+def test_spmv_pair_matches_oracle_and_is_adjoint(name):
+    lp = get_lp(name)
+    rng = np.random.default_rng(3)
+    x = rng.standard_normal(lp.n); y = rng.standard_normal(lp.m)
+    vs, _, _ = oracle.precondition(lp)
+    with P.UcLp(lp) as h:
+        kx = h.spmv(x, transpose=False)
+        kty = h.spmv(y, transpose=True)
+    ox, oty = oracle.spmv(lp, x, val=vs), oracle.spmv_t(lp, y, val=vs)
+    assert rel_l2(kx, ox) <= 1e-13 and rel_l2(kty, oty) <= 1e-13
+    assert abs(y @ kx - kty @ x) <= 1e-12 * (np.abs(y) @ np.abs(kx) + 1.0)       # adjoint identity
+
+
+# ------------------------------------------------------------------ R2..R11: 200-attempt trajectory
+@pytest.mark.parametrize("name", list(CASES))
+def test_trajectory_parity_200_attempts(name):
+    assert_trajectory_parity(get_lp(name), 200)
+
+
+def test_trajectory_parity_uc2_medium():
+    assert_trajectory_parity(uc_config(2), 200)
+
+
+@pytest.mark.parametrize("window,thr", [(32, 4), (64, 1), (100000, 1000)])
+def test_trajectory_parity_is_layout_independent(window, thr):
+    """Other slicing windows / long-row thresholds (all rows long, no row long) give the same iterates."""
+    assert_trajectory_parity(get_lp("ragged"), 130, sell_window=window, long_row_threshold=thr)
+
+
+def test_trajectory_parity_other_check_period_and_tail():
+    lp = get_lp("uc0")
+    for F, ce in ((37, 10), (64, 64), (65, 64), (1, 64)):
+        so = oracle.solve(lp, fixed_iterations=F, check_every=ce, trace_checks=64)
+        with P.UcLp(lp) as h:
+            sg = h.solve(fixed_iterations=F, check_every=ce, trace_checks=64)
+        assert rel_l2(sg.x, so.x) <= TOL_ITER and rel_l2(sg.y, so.y) <= TOL_ITER
+        np.testing.assert_array_equal(sg.checks["restart_kind"], so.checks["restart_kind"])
+        assert sg.iterations == F
+
+
+def test_warm_start_parity():
+    lp = get_lp("uc0")
+    rng = np.random.default_rng(9)
+    x0 = rng.uniform(-1, 2, lp.n); y0 = rng.standard_normal(lp.m)
+    so = oracle.solve(lp, x0=x0, y0=y0, fixed_iterations=100)
+    with P.UcLp(lp) as h:
+        sg = h.solve(x0=x0, y0=y0, fixed_iterations=100)
+    assert rel_l2(sg.x, so.x) <= TOL_ITER and rel_l2(sg.y, so.y) <= TOL_ITER
+
+
+# ------------------------------------------------------------------ convergence parity
+@pytest.mark.parametrize("name", ["two_var", "free_var", "small_random", "dispatch", "uc0"])
+def test_convergence_parity_live(name):
+    lp = get_lp(name)
+    so = oracle.solve(lp)
+    with P.UcLp(lp) as h:
+        sg = h.solve()
+    assert sg.status == P.OPTIMAL == so.status
+    assert sg.rel_kkt <= 1e-4
+    assert abs(sg.primal_obj - so.primal_obj) <= TOL_OBJ * (1 + abs(so.primal_obj))
+    assert abs(sg.dual_obj - so.dual_obj) <= TOL_OBJ * (1 + abs(so.dual_obj))
+    assert sg.iterations == so.iterations and sg.restarts == so.restarts and sg.returned_average == so.returned_average
+    k = oracle.kkt_unscaled(lp, sg.x, sg.y)              # the returned point really has that KKT error
+    assert k["rel_kkt"] == pytest.approx(sg.rel_kkt, rel=1e-6, abs=1e-12)
+    assert k["pobj"] == pytest.approx(sg.primal_obj, rel=1e-9)
+
+
+@pytest.mark.parametrize("i", [1, 2, 3])
+def test_convergence_parity_against_stored_oracle_runs(i):
+    """Configs 1-3 take the oracle 0.5 - 15 minutes: its results are stored by tests/golden/make_oracle_golden.py."""
+    gold = json.load(open(os.path.join(GOLDEN, "oracle_converged.json")))[f"uc_config{i}"]
+    lp = uc_config(i)
+    assert (lp.m, lp.n, lp.nnz) == (gold["m"], gold["n"], gold["nnz"])
+    with P.UcLp(lp) as h:
+        sg = h.solve(trace_checks=4096)
+    assert sg.status == P.OPTIMAL == gold["status"] and sg.rel_kkt <= 1e-4
+    assert abs(sg.primal_obj - gold["primal_obj"]) <= TOL_OBJ * abs(gold["primal_obj"])
+    assert abs(sg.dual_obj - gold["dual_obj"]) <= TOL_OBJ * abs(gold["dual_obj"])
+    assert abs(sg.iterations - gold["iterations"]) <= 0.1 * gold["iterations"]
+    k = oracle.kkt_unscaled(lp, sg.x, sg.y)
+    assert k["rel_kkt"] <= 1.0001e-4 and k["pobj"] == pytest.approx(sg.primal_obj, rel=1e-9)
+
+
+def test_converged_objective_matches_highs_on_config1():
+    lp = uc_config(1)
+    obj, _, _ = highs(lp)
+    with P.UcLp(lp) as h:
+        sg = h.solve()
+    assert abs(sg.primal_obj - obj) <= 1e-3 * (1 + abs(obj))
+
+
+# ------------------------------------------------------------------ full sizes of BASELINE.json
+def test_paper_scale_config3_trajectory_parity():
+    """Config 3 (6,049 buses, T=96) in the launch configuration bench.py times: 200 fixed attempts,
+    every element of x and y compared (the oracle needs ~0.1 s per attempt at this size)."""
+    sg, so = assert_trajectory_parity(uc_config(3), 200)
+    assert so.restarts >= 1
+
+
+@pytest.mark.parametrize("seed,F", [(10, 200), (11, 200), (12, 64)])
+def test_roofline_sweep_parity(seed, F):
+    from workloads import sweep_config
+    assert_trajectory_parity(sweep_config(seed), F)
+
+
+@pytest.mark.skipif(not os.environ.get("UC_PDHG_BIG"), reason="m = n = 1e7 / 2e7: set UC_PDHG_BIG=1 (minutes of host time, >20 GB host RAM)")
+@pytest.mark.parametrize("seed,F", [(13, 16), (14, 8)])
+def test_roofline_sweep_parity_largest(seed, F):
+    from workloads import sweep_config
+    assert_trajectory_parity(sweep_config(seed), F)
+
+
+# ------------------------------------------------------------------ degenerate inputs
+def test_empty_problem_and_no_columns():
+    z = np.zeros(0)
+    lp = LP(m=0, n=0, row_ptr=np.zeros(1, np.int64), col_idx=np.zeros(0, np.int32), val=z, sense=np.zeros(0, np.uint8),
+            b=z, c=z, l=z, u=z)
+    with P.UcLp(lp) as h:
+        s = h.solve(fixed_iterations=5)
+        assert s.iterations == 5 and s.x.size == 0
+        s = h.solve()
+        assert s.status == P.OPTIMAL
+    lp = LP(m=2, n=0, row_ptr=np.zeros(3, np.int64), col_idx=np.zeros(0, np.int32), val=z,
+            sense=np.full(2, ord("G"), np.uint8), b=-np.ones(2), c=z, l=z, u=z)
+    so = oracle.solve(lp, fixed_iterations=70)
+    with P.UcLp(lp) as h:
+        s = h.solve(fixed_iterations=70)
+    np.testing.assert_array_equal(s.y, so.y)
+
+
+def test_box_only_closed_form():
+    lp = tiny.box_only(n=40, seed=3)
+    with P.UcLp(lp) as h:
+        s = h.solve()
+    expect = np.where(lp.c > 0, lp.l, np.where(lp.c < 0, lp.u, np.clip(0.0, lp.l, lp.u)))
+    assert s.status == P.OPTIMAL
+    np.testing.assert_allclose(s.x, expect, atol=1e-9)
+
+
+def test_iteration_limit_returns_best_of_current_and_average():
+    lp = get_lp("uc0")
+    so = oracle.solve(lp, iter_limit=100)
+    with P.UcLp(lp) as h:
+        sg = h.solve(iter_limit=100)
+    assert sg.status == P.ITERATION_LIMIT == so.status and sg.iterations == 100
+    assert sg.returned_average == so.returned_average
+    assert rel_l2(sg.x, so.x) <= TOL_ITER and rel_l2(sg.y, so.y) <= TOL_ITER
+    assert sg.rel_kkt == pytest.approx(so.rel_kkt, rel=1e-6)
+
+
+def test_fixed_commitment_resolve_with_update_bounds():
+    lp = get_lp("uc0")
+    G, T, V, oU = lp.meta["G"], lp.meta["T"], lp.meta["V"], lp.meta["offsets"]["u"]
+    with P.UcLp(lp) as h:
+        relaxed = h.solve()
+        pattern = (relaxed.x.reshape(T, V)[:, oU:oU + G].T > 0.5).astype(float)
+        fixed = fix_commitment(lp, pattern)
+        so = oracle.solve(fixed)
+        h.update_bounds(fixed.l, fixed.u)
+        sg = h.solve()
+        h.update_bounds(lp.l, lp.u)
+        again = h.solve()
+    assert sg.status == P.OPTIMAL
+    assert abs(sg.primal_obj - so.primal_obj) <= TOL_OBJ * (1 + abs(so.primal_obj))
+    assert sg.iterations == so.iterations
+    assert sg.primal_obj >= relaxed.primal_obj * (1 - 2e-4)          # fixing u cannot improve the optimum
+    assert again.iterations == relaxed.iterations and again.primal_obj == relaxed.primal_obj
+
+
+def test_solves_are_reproducible_bit_for_bit():
+    lp = get_lp("uc1")
+    with P.UcLp(lp) as h:
+        a = h.solve(fixed_iterations=300)
+        b = h.solve(fixed_iterations=300)
+    with P.UcLp(lp) as h2:
+        c = h2.solve(fixed_iterations=300)
+    np.testing.assert_array_equal(a.x, b.x); np.testing.assert_array_equal(a.y, b.y)
+    np.testing.assert_array_equal(a.x, c.x); np.testing.assert_array_equal(a.y, c.y)
