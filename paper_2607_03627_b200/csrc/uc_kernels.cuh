@@ -207,22 +207,46 @@ __device__ __forceinline__ void sell_row(const Sell& A, int slice, int lane, dou
 }
 // Long-tail row r: the warp forms 32 products at a time (coalesced loads), then adds them in
 // entry order; the sums end up in every lane.
+// Memory latency, not the add chain, is what a long row costs (25 dependent round trips for 800 entries
+// if taken 32 at a time), so entries are taken 128 at a time and the (col, val) loads of the next batch
+// are in flight while the current batch is gathered and summed.
 template <int NV, class G>
 __device__ __forceinline__ void long_row(const Sell& A, int r, int lane, double (&s)[NV], G gather) {
+    constexpr int U = 4;
     const long long b = __ldg(A.lp + r), e = __ldg(A.lp + r + 1);
-    for (long long p0 = b; p0 < e; p0 += 32) {
-        const long long p = p0 + lane;
-        double prod[NV];
+    int cn[U]; double vn[U];
+    auto load_cv = [&](long long p0) {
 #pragma unroll
-        for (int q = 0; q < NV; ++q) prod[q] = 0.0;
-        if (p < e) {
-            int c = ld_stream(A.lcol + p); double v = ld_stream(A.lval + p); double g[NV];
-            gather(c, g);
-#pragma unroll
-            for (int q = 0; q < NV; ++q) prod[q] = __dmul_rn(v, g[q]);
+        for (int u = 0; u < U; ++u) {
+            const long long p = p0 + 32 * u + lane;
+            cn[u] = 0; vn[u] = 0.0;
+            if (p < e) { cn[u] = ld_stream(A.lcol + p); vn[u] = ld_stream(A.lval + p); }
         }
+    };
+    load_cv(b);
+    for (long long p0 = b; p0 < e; p0 += 32 * U) {
+        double prod[U][NV];
 #pragma unroll
-        for (int q = 0; q < NV; ++q) s[q] = warp_seq_add(s[q], prod[q]);
+        for (int u = 0; u < U; ++u) {                 // padding lanes gather column 0 and multiply by 0
+            double g[NV];
+            gather(cn[u], g);
+#pragma unroll
+            for (int q = 0; q < NV; ++q) prod[u][q] = g[q];
+        }
+        double v[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) v[u] = vn[u];
+        if (p0 + 32 * U < e) load_cv(p0 + 32 * U);
+#pragma unroll
+        for (int u = 0; u < U; ++u)
+#pragma unroll
+            for (int q = 0; q < NV; ++q) prod[u][q] = (p0 + 32 * u + lane < e) ? __dmul_rn(v[u], prod[u][q]) : 0.0;
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            if (p0 + 32 * u >= e) break;              // warp-uniform: whole chunk beyond the row end
+#pragma unroll
+            for (int q = 0; q < NV; ++q) s[q] = warp_seq_add(s[q], prod[u][q]);
+        }
     }
 }
 template <int NV, class G>
