@@ -8,7 +8,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libuc_pdhg.so")
 SOURCES = [os.path.join(CSRC, "uc_pdhg.cu")]
-DEPENDS = SOURCES + [os.path.join(CSRC, "uc_kernels.cuh"), os.path.join(CSRC, "uc_dd.cuh"), os.path.join(CSRC, "uc_format.hpp"),
+DEPENDS = SOURCES + [os.path.join(CSRC, "uc_kernels.cuh"), os.path.join(CSRC, "uc_attempt.cuh"), os.path.join(CSRC, "uc_dd.cuh"), os.path.join(CSRC, "uc_format.hpp"),
                      os.path.join(os.path.dirname(HERE), "include", "uc_pdhg.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-fmad=false", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared"]

@@ -28,7 +28,23 @@ struct HostSell {
     std::vector<int32_t> lcol;
     std::vector<double> lval;
     std::vector<int64_t> lsrc;
+    std::vector<int32_t> tile_ptr;    // [ntiles+1] first slice of each tile of the persistent attempt kernels
 };
+
+// Tiles of the persistent attempt kernels: consecutive slices, at most `max_slices` of them (one per
+// consumer warp) and at most `cap` stored entries in total (what one shared-memory stage holds).  A
+// single slice wider than `cap` forms a tile of its own (read straight from global memory).
+inline void build_tiles(HostSell& S, int max_slices, int64_t cap) {
+    S.tile_ptr.clear();
+    S.tile_ptr.push_back(0);
+    int64_t s = 0;
+    while (s < S.nslices) {
+        int64_t e = s + 1;
+        while (e < S.nslices && e - s < max_slices && S.slice_ptr[(size_t)e + 1] - S.slice_ptr[(size_t)s] <= cap) ++e;
+        S.tile_ptr.push_back((int32_t)e);
+        s = e;
+    }
+}
 
 // new -> old permutation: short rows in length-sorted windows, long rows last.
 inline void build_perm(const std::vector<int64_t>& len, int64_t window, int64_t long_thr,
@@ -168,5 +184,6 @@ inline void build_problem(int64_t m, int64_t n, int64_t nnz, const int64_t* row_
     }
     build_sell(n, tptr.data(), tidx.data(), tval.data(), tsrc.data(), P.perm_c, ns, P.inv_r, want_src, P.KT);
 }
+
 
 }  // namespace ucpdhg

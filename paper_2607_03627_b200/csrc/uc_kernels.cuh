@@ -65,6 +65,8 @@ struct Sell {
     int nlong;
     int nlblk;             // blocks covering the long tail = ceil(nlong / kWarps); they come FIRST in the grid
     int grid;              // nlblk + nblk, at least 1
+    const int* tile_ptr;   // [ntiles+1] first slice of each tile of the persistent attempt kernels (uc_attempt.cuh)
+    int ntiles;
 };
 
 struct Vecs {
@@ -76,12 +78,13 @@ struct Vecs {
     const double *c, *l, *u, *q; // scaled data
     const unsigned char* isG;
     const double *Dr, *Dc;
-    dd* partA;                   // [gridA]      sum dx^2
-    dd* partB;                   // [2][gridB]   sum dy^2, sum dy * (K dx)
+    dd* partA;                   // [gridPA]     sum dx^2            (one per CTA of the persistent primal kernel)
+    dd* partB;                   // [2][gridPB]  sum dy^2, sum dy * (K dx)
     dd* partD;                   // [8][gridA]   check, dual side
     dd* partP;                   // [6][gridB]   check, primal side
     dd* partR;                   // [2][gridR]   restart distances
-    int gridA, gridB, gridR;
+    int gridA, gridB, gridR;     // one-block-per-256-rows grids of the check / restart kernels
+    int gridPA, gridPB;          // persistent grids of the two attempt kernels
 };
 
 // ------------------------------------------------------------------------------------------ loads
@@ -253,107 +256,6 @@ template <int NV, class G>
 __device__ __forceinline__ void row_dot(const Sell& A, const RowId& r, int lane, double (&s)[NV], G gather) {
     if (r.slice >= 0) sell_row<NV>(A, r.slice, lane, s, gather);
     else long_row<NV>(A, r.lrow, lane, s, gather);
-}
-
-// ----------------------------------------------------------------- A5+A6 (+A10): primal kernel
-// g = K~' y ; x' = clamp(x - (eta/omega)(c - g), l, u) ; xbar = 2x' - x ; partial sum (x'-x)^2   (R3)
-// and, if the previous attempt was accepted, xsum += eta_prev * x  (R6, deferred by one attempt).
-__global__ void __launch_bounds__(kBlock) k_primal(Sell KT, Vecs V, Ctrl* ctl) {
-    __shared__ dd red[32];
-    if (ld_flag(&ctl->done)) return;
-    const int cur = ctl->cur, pend = ctl->pending;
-    const double eta_prev = ctl->eta_prev, tau = ctl->eta / ctl->omega;
-    const double* __restrict__ xcur = V.x[cur];
-    const double* __restrict__ ycur = V.y[cur];
-    double* __restrict__ xnext = V.x[cur ^ 1];
-    const int lane = threadIdx.x & 31;
-    const RowId r = my_row(KT);
-    dd acc[1] = {dd{0.0, 0.0}};
-    if (r.row >= 0) {
-        const long long j = r.row;
-        double xj = 0.0, cj = 0.0, lj = 0.0, uj = 0.0, xs = 0.0;
-        if (r.owner) {                       // own-vector loads first: in flight during the row dot
-            xj = xcur[j]; cj = V.c[j]; lj = V.l[j]; uj = V.u[j];
-            if (pend) xs = V.xsum[j];
-        }
-        double g[1] = {0.0};
-        row_dot<1>(KT, r, lane, g, [&](int c, double (&o)[1]) { o[0] = __ldg(ycur + c); });
-        if (r.owner) {
-            if (pend) V.xsum[j] = xs + eta_prev * xj;
-            const double v = xj - tau * (cj - g[0]);
-            const double xn = v < lj ? lj : (v > uj ? uj : v);
-            const double xb = 2.0 * xn - xj;
-            const double dx = xn - xj;
-            xnext[j] = xn;
-            V.xg[j] = make_double2(xb, dx);
-            acc[0].hi = dx * dx;
-        }
-    }
-    block_sum_dd<1>(acc, red);
-    if (threadIdx.x == 0) V.partA[blockIdx.x] = acc[0];
-}
-
-// ------------------------------------------------------------ A7+A8+A9 (+A10): dual kernel
-// r = K~ xbar ; y' = proj_Y(y + eta*omega (q - r)) ; partial sums dy^2 and dy.(K~ dx)   (R3, R4)
-// last block: finish the three reductions and run the step-size rule + accept test (R5).
-__global__ void __launch_bounds__(kBlock) k_dual(Sell K, Vecs V, Ctrl* ctl) {
-    __shared__ dd red[64];
-    if (ld_flag(&ctl->done)) return;
-    const int cur = ctl->cur, pend = ctl->pending;
-    const double eta_prev = ctl->eta_prev, sig = ctl->eta * ctl->omega;
-    const double* __restrict__ ycur = V.y[cur];
-    double* __restrict__ ynext = V.y[cur ^ 1];
-    const double2* __restrict__ xg = V.xg;
-    const int lane = threadIdx.x & 31;
-    const RowId r = my_row(K);
-    dd acc[2] = {dd{0.0, 0.0}, dd{0.0, 0.0}};
-    if (r.row >= 0) {
-        const long long i = r.row;
-        double yi = 0.0, qi = 0.0, ys = 0.0; int isg = 0;
-        if (r.owner) {
-            yi = ycur[i]; qi = V.q[i]; isg = V.isG[i];
-            if (pend) ys = V.ysum[i];
-        }
-        double kx[2] = {0.0, 0.0};               // K~ xbar, K~ dx
-        row_dot<2>(K, r, lane, kx, [&](int c, double (&o)[2]) { double2 t = __ldg(xg + c); o[0] = t.x; o[1] = t.y; });
-        if (r.owner) {
-            if (pend) V.ysum[i] = ys + eta_prev * yi;
-            const double v = yi + sig * (qi - kx[0]);
-            const double yn = (isg && v < 0.0) ? 0.0 : v;
-            const double dy = yn - yi;
-            ynext[i] = yn;
-            acc[0].hi = dy * dy; acc[1].hi = dy * kx[1];
-        }
-    }
-    block_sum_dd<2>(acc, red);
-    if (threadIdx.x == 0) { V.partB[blockIdx.x] = acc[0]; V.partB[V.gridB + blockIdx.x] = acc[1]; }
-    if (!last_block_done(&ctl->ticket_b)) return;
-
-    const dd sdx = final_sum(V.partA, V.gridA, red);
-    const dd sdy = final_sum(V.partB, V.gridB, red);
-    const dd sin_ = final_sum(V.partB + V.gridB, V.gridB, red);
-    if (threadIdx.x != 0) return;
-    ctl->ticket_b = 0;
-    const double dx2 = dd_round(sdx), dy2 = dd_round(sdy), inter = fabs(dd_round(sin_));
-    const double eta = ctl->eta, omega = ctl->omega;
-    const long long k = ctl->k + 1;
-    const double N = omega * dx2 + dy2 / omega;
-    const double eta_bar = (inter > 0.0) ? N / (2.0 * inter) : INFINITY;
-    const double2 pw = ctl->powtab[k - 1];                   // {(k+1)^-0.6, (k+1)^-0.3}
-    const double grow = (1.0 + pw.x) * eta;
-    const double eta_next = isinf(eta_bar) ? grow : fmin((1.0 - pw.y) * eta_bar, grow);
-    const int accept = eta <= eta_bar;
-    if (ctl->att && k - 1 < ctl->att_cap) {
-        uc_attempt_record rec;
-        rec.eta_used = eta; rec.eta_bar = eta_bar; rec.eta_next = eta_next;
-        rec.dx2 = dx2; rec.dy2 = dy2; rec.inter = inter; rec.accepted = accept; rec.pad_ = 0;
-        ctl->att[k - 1] = rec;
-    }
-    if (accept) { ctl->cur = cur ^ 1; ctl->pending = 1; ctl->eta_prev = eta; ctl->w += eta; ctl->accepted += 1; }
-    else ctl->pending = 0;
-    ctl->eta = eta_next;
-    ctl->k = k;
-    if (!isfinite(eta_next) || !(eta_next > 0.0)) { ctl->status = UC_NUMERICAL_ERROR; ctl->done = 1; }
 }
 
 // --------------------------------------------------------------------------- A10 flush before a check

@@ -12,6 +12,7 @@
 
 #include "uc_format.hpp"
 #include "uc_kernels.cuh"
+#include "uc_attempt.cuh"
 
 using namespace ucpdhg;
 
@@ -73,14 +74,17 @@ struct uc_lp {
     // host permutations (for warm starts / hooks)
     std::vector<int64_t> h_perm_r, h_perm_c;
 
+    // every array gets one slice (32 elements) of zeroed slack: the bulk copies of the attempt kernels read
+    // whole 32-row segments, and the last slice of the sliced part may be ragged
     template <class T>
     T* dalloc(size_t count) {
         void* p = nullptr;
-        size_t bytes = (count ? count : 1) * sizeof(T);
+        size_t bytes = (count + 32) * sizeof(T);
         cudaError_t e = cudaMalloc(&p, bytes);
         if (e != cudaSuccess) throw CudaFail{e, "cudaMalloc"};
         allocs.push_back(p);
         device_bytes += bytes;
+        if (cudaMemset(p, 0, bytes) != cudaSuccess) throw CudaFail{cudaGetLastError(), "cudaMemset"};
         return (T*)p;
     }
     template <class T>
@@ -113,6 +117,8 @@ Sell upload_sell(uc_lp* lp, const HostSell& H) {
     S.nlblk = cdiv(H.nlong, kWarps);
     S.grid = S.nlblk + S.nblk;
     if (S.grid < 1) S.grid = 1;
+    S.tile_ptr = lp->upload(H.tile_ptr);
+    S.ntiles = (int)H.tile_ptr.size() - 1;
     return S;
 }
 
@@ -166,8 +172,8 @@ void ensure_powtab(uc_lp* lp, long long limit) {
 }
 
 void launch_attempt(uc_lp* lp, cudaStream_t st) {
-    k_primal<<<lp->KT.grid, kBlock, 0, st>>>(lp->KT, lp->V, lp->ctl);
-    k_dual<<<lp->K.grid, kBlock, 0, st>>>(lp->K, lp->V, lp->ctl);
+    k_primal<<<lp->V.gridPA, kAttemptThreads, sizeof(PrimalPipe), st>>>(lp->KT, lp->V, lp->ctl);
+    k_dual<<<lp->V.gridPB, kAttemptThreads, sizeof(DualPipe), st>>>(lp->K, lp->V, lp->ctl);
 }
 void launch_kkt(uc_lp* lp, cudaStream_t st, int mode) {
     k_check_dual<<<lp->KT.grid, kBlock, 0, st>>>(lp->KT, lp->V, lp->ctl);
@@ -298,6 +304,8 @@ int uc_lp_create(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, cons
         // A0 / A1: layouts (host), upload
         HostProblem P;
         build_problem(m, n, nnz, row_ptr, col_idx, val, opt.sell_window, opt.long_row_threshold, opt.keep_source_map != 0, P);
+        build_tiles(P.K, kCons, kCap);
+        build_tiles(P.KT, kCons, kCap);
         lp->K = upload_sell(lp, P.K);
         lp->KT = upload_sell(lp, P.KT);
         lp->k_slots = (int64_t)P.K.col.size(); lp->kt_slots = (int64_t)P.KT.col.size();
@@ -318,8 +326,17 @@ int uc_lp_create(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, cons
         lp->Dr = lp->dalloc<double>((size_t)m); lp->Dc = lp->dalloc<double>((size_t)n);
         V.c = lp->cs; V.l = lp->ls; V.u = lp->us; V.q = lp->qs; V.isG = lp->isG; V.Dr = lp->Dr; V.Dc = lp->Dc;
         V.gridA = lp->KT.grid; V.gridB = lp->K.grid; V.gridR = std::max(1, cdiv(n + m, kBlock));
-        V.partA = lp->dalloc<dd>((size_t)V.gridA);
-        V.partB = lp->dalloc<dd>((size_t)2 * V.gridB);
+        {   // persistent grids of the attempt kernels: kCtasPerSm CTAs per SM, never more CTAs than work items
+            int sms = 0;
+            CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+            const int cap = kCtasPerSm * std::max(sms, 1);
+            V.gridPA = std::max(1, std::min(cap, std::max(lp->KT.ntiles, lp->KT.nlong)));
+            V.gridPB = std::max(1, std::min(cap, std::max(lp->K.ntiles, lp->K.nlong)));
+            CK(cudaFuncSetAttribute(k_primal, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(PrimalPipe)));
+            CK(cudaFuncSetAttribute(k_dual, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(DualPipe)));
+        }
+        V.partA = lp->dalloc<dd>((size_t)V.gridPA);
+        V.partB = lp->dalloc<dd>((size_t)2 * V.gridPB);
         V.partD = lp->dalloc<dd>((size_t)8 * V.gridA);
         V.partP = lp->dalloc<dd>((size_t)6 * V.gridB);
         V.partR = lp->dalloc<dd>((size_t)2 * V.gridR);
@@ -559,9 +576,9 @@ int uc_pdhg_time_kernels(uc_lp* lp, void* stream, int32_t attempts, double* prim
         for (auto& e : ev) CK(cudaEventCreate(&e));
         CK(cudaEventRecord(ev[0], st));
         for (int i = 0; i < attempts; ++i) {
-            k_primal<<<lp->KT.grid, kBlock, 0, st>>>(lp->KT, lp->V, lp->ctl);
+            k_primal<<<lp->V.gridPA, kAttemptThreads, sizeof(PrimalPipe), st>>>(lp->KT, lp->V, lp->ctl);
             CK(cudaEventRecord(ev[(size_t)2 * i + 1], st));
-            k_dual<<<lp->K.grid, kBlock, 0, st>>>(lp->K, lp->V, lp->ctl);
+            k_dual<<<lp->V.gridPB, kAttemptThreads, sizeof(DualPipe), st>>>(lp->K, lp->V, lp->ctl);
             CK(cudaEventRecord(ev[(size_t)2 * i + 2], st));
         }
         CK(cudaStreamSynchronize(st));
