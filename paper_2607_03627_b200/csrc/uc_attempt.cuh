@@ -6,22 +6,33 @@
 //                          dy.(K~ dx) ; the last CTA finishes the three reductions and runs the
 //                          step-size rule and the accept test                              (R3..R5)
 //
-// Both are HBM-bound streams (0.16 flop/B), so the design question is only how to keep ~45 KB per SM in
-// flight with 3.4 entries per row.  Answer: persistent, warp-specialised CTAs, two per SM, each with
-//   * one PRODUCER warp: for every tile (<= 8 slices = 256 rows, <= kCap stored entries) it issues 1-D
-//     TMA bulk copies (cp.async.bulk ... mbarrier::complete_tx) of everything the tile streams -- the
-//     column indices and values of its slices (one contiguous span of the sliced-ELL arrays) and the
-//     256-row segments of the per-row vectors -- into a ring of kStages shared-memory stages, up to
-//     kStages tiles ahead of the consumers;
-//   * kCons CONSUMER warps: warp w owns slice w of the tile, one thread per row; it waits on the
-//     stage's full-barrier, reads its operands from shared memory, gathers the other vector
-//     (y, or the pair {xbar, dx}) from L2 with up to four loads in flight, forms the row sum left to
-//     right, applies the update, stores coalesced, and releases the stage;
-//   * one LONG-ROW warp: rows longer than the sliced-ELL threshold (the T reserve rows of the UC LP),
-//     one row at a time, concurrently with the tile pipeline.
-// Tiles are dealt round-robin (tile = blockIdx.x + i * gridDim.x).  Every thread keeps its
-// double-double partial sums in registers across all its tiles; there is ONE block reduction per
-// kernel, then one partial per CTA, and the last CTA to finish (ticket) adds the <= 2 * #SM partials.
+// Both are HBM-bound streams (0.16 flop/B) of rows with ~3.4 entries, each entry needing an irregular
+// 8/16-byte gather.  The design question is how to keep ~50 KB per SM in flight AND issue ~45k gathers per
+// SM per kernel.  What was measured on B200 (profiles/):
+//   * a 1-D TMA bulk copy (cp.async.bulk) costs its issuing thread ~160 cycles whatever its size -- right for
+//     16 KB tiles, hopeless for the 2 KB vector segments and ~1 KB index/value chunks this path is made of;
+//   * a coalesced cp.async (LDGSTS.128) costs ~8 cycles and holds no register while in flight;
+//   * divergent gathers run at ~1000 gathers/us/SM from 4 issuing warps but ~1500 from 8 or more.
+// Hence: persistent CTAs (two per SM) of kAttWarps CONSUMER warps, every one of which runs its own
+// three-deep software pipeline on its own shared-memory rings, with NO block-level synchronisation inside
+// the loop.  The unit of work is a STEP (uc_format.hpp): up to kChunkT entries per row of one slice (32 rows,
+// one per lane).  For its step j a warp has, in flight at the same time,
+//     A(j + kDA): cp.async of the step's column indices                         -> index ring
+//     B(j + kDB): cp.async of the step's matrix values, of the 32-row segments of the per-row vectors
+//                 (last step of a slice only) and, using the indices that A brought in, one 8/16-byte
+//                 cp.async per stored entry e:  gv[e] <- src[col[e]]  (the entry of y, or of the pair
+//                 {xbar, dx}, that e multiplies)                                -> data ring
+//     C(j):       everything read from shared memory: row sums left to right, update, coalesced stores.
+// One cp.async group is committed per step; cp.async.wait_group kDB + __syncwarp is the only wait.  A slice
+// wider than kChunkT is a run of consecutive steps whose row sums stay in registers.  The schedule (slice s ->
+// warp s % #warps, built at create time) is static, so results are reproducible bit for bit.  One extra warp
+// per CTA takes the rows longer than the sliced-ELL threshold (the T reserve rows of the UC LP), one row at a
+// time, concurrently.
+// L2 policy: streamed-once data is loaded (cp.async.cg, L1 bypass) and stored evict_first; the gathered vectors
+// (y', {xbar, dx}) are stored evict_last so that the gathers of the NEXT kernel hit in the 126 MB L2.
+// Every thread keeps its double-double partial sums in registers across all its steps; there is ONE block
+// reduction per kernel, then one partial per CTA, and the last CTA to finish (ticket) adds the <= 2 * #SM
+// partials.
 //
 // Arithmetic is unchanged from the sequential statement: row sums left to right in CSR order, multiply
 // and add rounded separately (-fmad=false), long reductions in double-double (order-independent once
@@ -31,167 +42,183 @@
 
 namespace ucpdhg {
 
-constexpr int kCons = 8;                       // consumer warps per CTA = slices per tile
-constexpr int kAttemptThreads = (kCons + 2) * 32;   // + producer warp + long-row warp
-constexpr int kStages = 3;                     // shared-memory stages per CTA
-constexpr int kCap = 2048;                     // stored matrix entries one stage can hold
-constexpr int kTileRows = kCons * 32;
-constexpr int kCtasPerSm = 2;
+// build-time tunables (-DUC_...): the defaults are the measured optimum on config 3 (profiles/)
+#ifndef UC_ATT_WARPS
+#define UC_ATT_WARPS 7
+#endif
+#ifndef UC_CTAS_PER_SM
+#define UC_CTAS_PER_SM 2
+#endif
+#ifndef UC_DB
+#define UC_DB 1
+#endif
+constexpr int kAttWarps = UC_ATT_WARPS;        // consumer warps per CTA
+constexpr int kCtasPerSm = UC_CTAS_PER_SM;
+constexpr int kAttemptThreads = (kAttWarps + 1) * 32;   // + long-row warp
+constexpr int kDB = UC_DB;                     // data (values, vectors, gathers) run kDB steps ahead of the compute
+constexpr int kDA = 2 * kDB + 1;               // indices run kDA steps ahead: a group is complete kDB commits later
+constexpr int kRingA = kDA - kDB + 1;          // slots of the index ring
+constexpr int kRingB = kDB + 1;                // slots of the data ring
+constexpr int kChunkE = kChunkT * 32;          // stored entries per step
 
 // ------------------------------------------------------------------------------------------ PTX
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+// L2 eviction policies (createpolicy): streamed-once data leaves L2 first, gathered vectors last
+__device__ __forceinline__ uint64_t policy_evict_first() {
+    uint64_t p; asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p)); return p;
 }
-__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+__device__ __forceinline__ uint64_t policy_evict_last() {
+    uint64_t p; asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p)); return p;
 }
-__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+// asynchronous global -> shared copies (LDGSTS): no destination register; completion per thread, by group.
+// 16-byte streaming copy, L1 bypass, evict_first in L2
+__device__ __forceinline__ void cp_stream16(void* dst, const void* src, uint64_t pol) {
+    asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2;" ::"r"(smem_u32(dst)), "l"(src), "l"(pol) : "memory");
 }
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-    asm volatile(
-        "{\n"
-        ".reg .pred P1;\n"
-        "LAB_WAIT:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
-        "@P1 bra DONE;\n"
-        "bra LAB_WAIT;\n"
-        "DONE:\n"
-        "}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+// 8 / 16-byte gather
+__device__ __forceinline__ void cp_gather(double* dst, const double* src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
 }
-// 1-D TMA bulk copy global -> shared, completion counted in bytes on `bar`.  dst, src and bytes are
-// multiples of 16.
-__device__ __forceinline__ void tma_load(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
-                 "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+__device__ __forceinline__ void cp_gather(double2* dst, const double2* src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"(src) : "memory");   // L1 bypass: measured faster
 }
-__device__ __forceinline__ void fence_barrier_init() {
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+__device__ __forceinline__ void cp_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+__device__ __forceinline__ void st_hint(double* p, double v, uint64_t pol) {
+    asm volatile("st.global.L2::cache_hint.f64 [%0], %1, %2;" ::"l"(p), "d"(v), "l"(pol) : "memory");
 }
+__device__ __forceinline__ void st_hint(double2* p, double2 v, uint64_t pol) {
+    asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1, %2}, %3;" ::"l"(p), "d"(v.x), "d"(v.y), "l"(pol) : "memory");
+}
+struct Policies { uint64_t first, last; };
 
-// ------------------------------------------------------------------------------------------ stage
-struct StageHdr {
-    long long span_base;     // first stored entry of the tile in the sliced-ELL arrays
-    int first_slice, nslices, staged, pad;
-    int woff[kCons + 1];     // entry offset of each slice inside the span
-    int pad2;
+// ------------------------------------------------------------------------------------------ per-warp rings
+// GT: what one entry gathers -- double (y) or double2 ({xbar, dx}).  Everything in here is private to ONE warp.
+template <int NVEC, bool BYTEVEC, class GT>
+struct DataSlot {
+    double val[kChunkE];
+    GT gv[kChunkE];              // gv[e] = gathered vector entry for stored entry e
+    double vec[NVEC][32];        // 32-row segments of the per-row vectors (last step of a slice only)
+    unsigned char bvec[BYTEVEC ? 32 : 16];
 };
-static_assert(sizeof(StageHdr) == 64, "StageHdr layout");
-
-template <int NVEC, bool BYTEVEC>
-struct StageT {
-    StageHdr hdr;
-    int col[kCap];
-    double val[kCap];
-    double vec[NVEC][kTileRows];
-    unsigned char bvec[BYTEVEC ? kTileRows : 16];
+template <int NVEC, bool BYTEVEC, class GT>
+struct WarpRing {
+    int col[kRingA][kChunkE];
+    DataSlot<NVEC, BYTEVEC, GT> data[kRingB];
 };
-template <int NVEC, bool BYTEVEC>
-struct PipeT {
-    StageT<NVEC, BYTEVEC> st[kStages];
-    uint64_t full[kStages], empty[kStages];
+template <int NVEC, bool BYTEVEC, class GT>
+struct SmemT {
+    WarpRing<NVEC, BYTEVEC, GT> w[kAttWarps];
     dd red[2 * 32];
     int is_last;
 };
-using PrimalPipe = PipeT<5, false>;   // x, c, l, u, xsum
-using DualPipe = PipeT<3, true>;      // y, q, ysum + isG
+using PrimalSmem = SmemT<5, false, double>;   // x, c, l, u, xsum ; gathers y
+using DualSmem = SmemT<3, true, double2>;     // y, q, ysum + isG ; gathers {xbar, dx}
+static_assert(kCtasPerSm * (sizeof(PrimalSmem) + 1024) <= 228 * 1024 && kCtasPerSm * (sizeof(DualSmem) + 1024) <= 228 * 1024,
+              "the CTAs of either attempt kernel must fit the shared memory of one SM");
 
-// ------------------------------------------------------------------------------------------ producer
-// One warp.  For tile i of this CTA: wait until the consumers have released stage i % kStages, write the
-// tile header, arm the full-barrier with the byte count and issue the bulk copies.  `vec_copies(stage,
-// row0, rows, bar)` issues the per-row vector copies and returns their byte count.  The tile's slice
-// pointers are loaded one tile ahead so that their latency hides behind the wait.
-template <class Pipe, class VC>
-__device__ __forceinline__ void producer_loop(const Sell& A, Pipe& P, int lane, VC vec_copies) {
-    int t = blockIdx.x;
-    int fs = 0, ns = 0; long long spv = 0;
-    auto fetch = [&](int tile) {
-        fs = __ldg(A.tile_ptr + tile); ns = __ldg(A.tile_ptr + tile + 1) - fs;
-        spv = (lane <= ns) ? __ldg(A.sp + fs + lane) : 0;
+// ------------------------------------------------------------------------------------------ the pipeline
+// Runs the steps of consumer warp `gw` (of A.sched_warps) through the A / B / C pipeline described at the top.
+//   issue_vecs(slot, row0)    issues the cp.async copies of the 32-row vector segments of a slice
+//   compute(slot, info, row0) consumes one step from shared memory
+// The schedule is read 32 steps at a time (lane l holds step 32 b + l of the warp; the next batch is loaded
+// one batch ahead) and a step's descriptor travels from A to B to C through two small register queues, so
+// only the A cursor ever touches it.
+template <class Ring, class GT, class FV, class FC>
+__device__ __forceinline__ void warp_pipeline(const Sell& A, Ring& R, int gw, int lane, const GT* __restrict__ gsrc,
+                                              uint64_t pol_first, FV issue_vecs, FC compute) {
+    const int J = A.steps_per_warp;
+    const long long GW = A.sched_warps;
+    auto load_desc = [&](int k) -> int4 {
+        return k < J ? __ldg(reinterpret_cast<const int4*>(A.steps + (long long)k * GW + gw)) : make_int4(0, 0, 0, 0);
     };
-    if (t < A.ntiles) fetch(t);
-    for (int i = 0; t < A.ntiles; ++i, t += gridDim.x) {
-        const int s = i % kStages;
-        const uint32_t ph = (uint32_t)(i / kStages) & 1u;
-        const int cfs = fs, cns = ns; const long long cspv = spv;
-        if (t + (int)gridDim.x < A.ntiles) fetch(t + gridDim.x);
-        mbar_wait(&P.empty[s], ph ^ 1u);
-        auto& S = P.st[s];
-        const long long base = __shfl_sync(0xffffffffu, cspv, 0);
-        const int span = (int)(__shfl_sync(0xffffffffu, cspv, cns) - base);
-        const int staged = span <= kCap;
-        if (lane <= cns) S.hdr.woff[lane] = (int)(cspv - base);
-        if (lane == 0) { S.hdr.span_base = base; S.hdr.first_slice = cfs; S.hdr.nslices = cns; S.hdr.staged = staged; }
-        __syncwarp();
-        if (lane == 0) {
-            const long long row0 = 32LL * cfs; const int rows = 32 * cns;
-            uint32_t bytes = vec_copies(S, row0, rows, (uint64_t*)nullptr);       // count only
-            if (staged) bytes += 12u * (uint32_t)span;
-            mbar_expect_tx(&P.full[s], bytes);
-            vec_copies(S, row0, rows, &P.full[s]);
-            if (staged && span > 0) {
-                tma_load(S.col, A.col + base, 4u * (uint32_t)span, &P.full[s]);
-                tma_load(S.val, A.val + base, 8u * (uint32_t)span, &P.full[s]);
+    int4 dcur = load_desc(lane), dnxt = load_desc(32 + lane);
+    long long qa_e[kDA - kDB]; int qa_i[kDA - kDB], qa_r[kDA - kDB];     // A -> B
+    int qb_i[kDB], qb_r[kDB];                                            // B -> C
+#pragma unroll
+    for (int q = 0; q < kDA - kDB; ++q) { qa_e[q] = 0; qa_i[q] = 0; qa_r[q] = 0; }
+#pragma unroll
+    for (int q = 0; q < kDB; ++q) { qb_i[q] = 0; qb_r[q] = 0; }
+    // ring slots of steps ka (index ring), kb (index ring: kb = ka - (kRingA - 1)), kb (data ring: kb = -kRingB at the start), j
+    int sa = 0, sbA = 1 % kRingA, sb = 0, sc = 0;
+    for (int j = -kDA; j < J; ++j) {
+        // ---- A: column indices of step ka = j + kDA
+        const int ka = j + kDA;
+        if (ka >= 32 && (ka & 31) == 0) { dcur = dnxt; dnxt = load_desc(ka + 32 + lane); }
+        const int src_lane = ka & 31;
+        const int dx_ = __shfl_sync(0xffffffffu, dcur.x, src_lane), dy_ = __shfl_sync(0xffffffffu, dcur.y, src_lane);
+        const int row_a = __shfl_sync(0xffffffffu, dcur.z, src_lane), info_a = __shfl_sync(0xffffffffu, dcur.w, src_lane);
+        const long long eb_a = ((long long)(unsigned)dx_) | ((long long)dy_ << 32);
+        if (lane < (info_a & 7) * 8) cp_stream16(&R.col[sa][lane * 4], A.col + eb_a + lane * 4, pol_first);
+        // ---- B: values, vectors and gathers of step kb = j + kDB (its indices landed kDB commits ago)
+        const long long eb = qa_e[0]; const int info_b = qa_i[0], row_b = qa_r[0];
+#pragma unroll
+        for (int q = 0; q + 1 < kDA - kDB; ++q) { qa_e[q] = qa_e[q + 1]; qa_i[q] = qa_i[q + 1]; qa_r[q] = qa_r[q + 1]; }
+        qa_e[kDA - kDB - 1] = eb_a; qa_i[kDA - kDB - 1] = info_a; qa_r[kDA - kDB - 1] = row_a;
+        {
+            const int nt = info_b & 7;
+            auto& D = R.data[sb];
+#pragma unroll
+            for (int k = 0; k < kChunkT / 2; ++k) {
+                const int p = k * 32 + lane;                       // 16-byte piece of the value chunk
+                if (p < nt * 16) cp_stream16(&D.val[p * 2], A.val + eb + p * 2, pol_first);
             }
+            if (info_b & 32) issue_vecs(D, row_b);
+#pragma unroll
+            for (int t = 0; t < kChunkT; ++t)
+                if (t < nt) cp_gather(&D.gv[t * 32 + lane], gsrc + R.col[sbA][t * 32 + lane]);
         }
-        __syncwarp();
+        cp_commit();
+        // ---- C: step j
+        const int info_c = qb_i[0], row_c = qb_r[0];
+#pragma unroll
+        for (int q = 0; q + 1 < kDB; ++q) { qb_i[q] = qb_i[q + 1]; qb_r[q] = qb_r[q + 1]; }
+        qb_i[kDB - 1] = info_b; qb_r[kDB - 1] = row_b;
+        cp_wait<kDB>();
+        __syncwarp();                                              // the copies of every lane are visible to the warp
+        if (info_c) compute(R.data[sc], info_c, row_c);
+        __syncwarp();                                              // slots are rewritten by the next iteration's copies
+        sa = (sa + 1 == kRingA) ? 0 : sa + 1; sbA = (sbA + 1 == kRingA) ? 0 : sbA + 1;
+        sb = (sb + 1 == kRingB) ? 0 : sb + 1;
+        if (j >= 0) sc = (sc + 1 == kRingB) ? 0 : sc + 1;
     }
+    cp_wait<0>();
 }
 
-template <class Pipe>
-__device__ __forceinline__ void pipe_init(Pipe& P) {
-    if (threadIdx.x == 0) {
+// Row sum contribution of one step: entries t*32+lane of the slot, t = 0..nt-1, left to right.
+template <int NV, class GT>
+__device__ __forceinline__ void step_sum(const double* valp, const GT* gvp, int nt, int lane, double (&s)[NV]) {
+    double v[kChunkT]; GT g[kChunkT];
 #pragma unroll
-        for (int s = 0; s < kStages; ++s) { mbar_init(&P.full[s], 1); mbar_init(&P.empty[s], kCons); }
-        fence_barrier_init();
-    }
-    __syncthreads();
-}
-
-// Row sum of one sliced-ELL row from (colp, valp) -- either the shared-memory stage or, for a tile that
-// did not fit a stage, global memory -- entries t*32+lane, t = 0..width-1, left to right.  Four gathers
-// are in flight at a time; slots past the width are not added.
-template <int NV, class CP, class VP, class G>
-__device__ __forceinline__ void slice_row(CP colp, VP valp, int width, int lane, double (&s)[NV], G gather) {
-    for (int t = 0; t < width; t += 4) {
-        int c[4]; double v[4]; double g[4][NV];
+    for (int t = 0; t < kChunkT; ++t)
+        if (t < nt) { v[t] = valp[t * 32 + lane]; g[t] = gvp[t * 32 + lane]; }
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            const bool ok = t + u < width;
-            c[u] = ok ? colp[(t + u) * 32 + lane] : 0;
-            v[u] = ok ? valp[(t + u) * 32 + lane] : 0.0;
+    for (int t = 0; t < kChunkT; ++t)
+        if (t < nt) {
+            if constexpr (NV == 1) s[0] = __dadd_rn(s[0], __dmul_rn(v[t], g[t]));
+            else { s[0] = __dadd_rn(s[0], __dmul_rn(v[t], g[t].x)); s[1] = __dadd_rn(s[1], __dmul_rn(v[t], g[t].y)); }
         }
-#pragma unroll
-        for (int u = 0; u < 4; ++u) gather(c[u], g[u]);
-#pragma unroll
-        for (int u = 0; u < 4; ++u)
-            if (t + u < width) {
-#pragma unroll
-                for (int q = 0; q < NV; ++q) s[q] = __dadd_rn(s[q], __dmul_rn(v[u], g[u][q]));
-            }
-    }
 }
 
 // ----------------------------------------------------------------- A5+A6 (+A10): primal kernel
 // One row j of K~' (= variable j): given g = (K~'y)_j, the R3 update and the R6 deferred average.
 struct PrimalRow { double x, c, l, u, xs; };
 __device__ __forceinline__ double primal_update(const Vecs& V, double* __restrict__ xnext, long long j, const PrimalRow& r,
-                                                double g, double tau, int pend, double eta_prev) {
-    if (pend) V.xsum[j] = r.xs + eta_prev * r.x;
+                                                double g, double tau, int pend, double eta_prev, const Policies& pol) {
+    if (pend) st_hint(V.xsum + j, r.xs + eta_prev * r.x, pol.first);
     const double v = r.x - tau * (r.c - g);
     const double xn = v < r.l ? r.l : (v > r.u ? r.u : v);
     const double xb = 2.0 * xn - r.x;
     const double dx = xn - r.x;
-    xnext[j] = xn;
-    V.xg[j] = make_double2(xb, dx);
+    st_hint(xnext + j, xn, pol.first);
+    st_hint(V.xg + j, make_double2(xb, dx), pol.last);      // gathered by the next k_dual: keep it in L2
     return dx * dx;
 }
 
 __global__ void __launch_bounds__(kAttemptThreads, kCtasPerSm) k_primal(Sell KT, Vecs V, Ctrl* ctl) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    PrimalPipe& P = *reinterpret_cast<PrimalPipe*>(smem_raw);
+    PrimalSmem& P = *reinterpret_cast<PrimalSmem*>(smem_raw);
     if (ld_flag(&ctl->done)) return;
     const int cur = ctl->cur, pend = ctl->pending;
     const double eta_prev = ctl->eta_prev, tau = ctl->eta / ctl->omega;
@@ -199,53 +226,45 @@ __global__ void __launch_bounds__(kAttemptThreads, kCtasPerSm) k_primal(Sell KT,
     const double* __restrict__ ycur = V.y[cur];
     double* __restrict__ xnext = V.x[cur ^ 1];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    pipe_init(P);
     dd acc[1] = {dd{0.0, 0.0}};
+    const Policies pol{policy_evict_first(), policy_evict_last()};
 
-    if (warp == kCons) {                                   // ---- producer
-        producer_loop(KT, P, lane, [&](auto& S, long long row0, int rows, uint64_t* bar) -> uint32_t {
-            const uint32_t b = 8u * (uint32_t)rows;
-            if (bar) {
-                tma_load(S.vec[0], xcur + row0, b, bar);
-                tma_load(S.vec[1], V.c + row0, b, bar);
-                tma_load(S.vec[2], V.l + row0, b, bar);
-                tma_load(S.vec[3], V.u + row0, b, bar);
-                if (pend) tma_load(S.vec[4], V.xsum + row0, b, bar);
-            }
-            return (pend ? 5u : 4u) * b;
-        });
-    } else if (warp == kCons + 1) {                        // ---- long rows, one per pass
+    if (warp == kAttWarps) {                               // ---- long rows, one per pass
         for (int r = blockIdx.x; r < KT.nlong; r += gridDim.x) {
             const long long j = KT.nshort + r;
             PrimalRow pr{0.0, 0.0, 0.0, 0.0, 0.0};
             if (lane == 0) { pr.x = xcur[j]; pr.c = V.c[j]; pr.l = V.l[j]; pr.u = V.u[j]; if (pend) pr.xs = V.xsum[j]; }
             double g[1] = {0.0};
             long_row<1>(KT, r, lane, g, [&](int c, double (&o)[1]) { o[0] = __ldg(ycur + c); });
-            if (lane == 0) acc[0] = dd_add_d(acc[0], primal_update(V, xnext, j, pr, g[0], tau, pend, eta_prev));
+            if (lane == 0) acc[0] = dd_add_d(acc[0], primal_update(V, xnext, j, pr, g[0], tau, pend, eta_prev, pol));
         }
-    } else {                                               // ---- consumers: warp w owns slice w of each tile
-        int t = blockIdx.x;
-        for (int i = 0; t < KT.ntiles; ++i, t += gridDim.x) {
-            const int s = i % kStages;
-            mbar_wait(&P.full[s], (uint32_t)(i / kStages) & 1u);
-            auto& S = P.st[s];
-            if (warp < S.hdr.nslices) {
-                const long long j = 32LL * (S.hdr.first_slice + warp) + lane;
-                const int r = warp * 32 + lane;
-                const int off = S.hdr.woff[warp], width = (S.hdr.woff[warp + 1] - off) >> 5;
-                PrimalRow pr{S.vec[0][r], S.vec[1][r], S.vec[2][r], S.vec[3][r], pend ? S.vec[4][r] : 0.0};
-                double g[1] = {0.0};
-                auto gather = [&](int c, double (&o)[1]) { o[0] = __ldg(ycur + c); };
-                if (S.hdr.staged) slice_row<1>(S.col + off, S.val + off, width, lane, g, gather);
-                else slice_row<1>(KT.col + S.hdr.span_base + off, (const double*)KT.val + S.hdr.span_base + off, width, lane, g, gather);
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&P.empty[s]);
-                if (j < KT.nshort) acc[0] = dd_add_d(acc[0], primal_update(V, xnext, j, pr, g[0], tau, pend, eta_prev));
-            } else {
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&P.empty[s]);
-            }
+    } else {                                               // ---- consumer warps
+        double g[1] = {0.0};
+        // this lane's share of a slice's vector segments: piece k covers vector v = 2k + lane/16, doubles off, off+1
+        const double* vsrc[3]; int voff[3]; bool vok[3];
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const int v = 2 * k + (lane >> 4), off = (lane & 15) * 2;
+            vsrc[k] = (v == 0 ? xcur : v == 1 ? V.c : v == 2 ? V.l : v == 3 ? V.u : V.xsum) + off;
+            voff[k] = v * 32 + off; vok[k] = v < 4 || (v == 4 && pend);
         }
+        warp_pipeline(KT, P.w[warp], (int)blockIdx.x * kAttWarps + warp, lane, ycur, pol.first,
+            [&](auto& D, int row0) {                       // x, c, l, u (, xsum): 16 pieces of 16 bytes each
+#pragma unroll
+                for (int k = 0; k < 3; ++k)
+                    if (vok[k]) cp_stream16(&D.vec[0][0] + voff[k], vsrc[k] + row0, pol.first);
+            },
+            [&](auto& D, int info, int row0) {
+                if (info & 16) g[0] = 0.0;
+                step_sum<1>(D.val, D.gv, info & 7, lane, g);
+                if (info & 32) {
+                    const long long j = (long long)row0 + lane;
+                    if (j < KT.nshort) {
+                        const PrimalRow pr{D.vec[0][lane], D.vec[1][lane], D.vec[2][lane], D.vec[3][lane], pend ? D.vec[4][lane] : 0.0};
+                        acc[0] = dd_add_d(acc[0], primal_update(V, xnext, j, pr, g[0], tau, pend, eta_prev, pol));
+                    }
+                }
+            });
     }
     block_sum_dd<1>(acc, P.red);
     if (threadIdx.x == 0) V.partA[blockIdx.x] = acc[0];
@@ -255,17 +274,17 @@ __global__ void __launch_bounds__(kAttemptThreads, kCtasPerSm) k_primal(Sell KT,
 struct DualRow { double y, q, ys; int isg; };
 // kx[0] = (K~ xbar)_i, kx[1] = (K~ dx)_i.  Returns dy; the caller accumulates dy^2 and dy * kx[1].
 __device__ __forceinline__ double dual_update(const Vecs& V, double* __restrict__ ynext, long long i, const DualRow& r,
-                                              const double (&kx)[2], double sig, int pend, double eta_prev) {
-    if (pend) V.ysum[i] = r.ys + eta_prev * r.y;
+                                              const double (&kx)[2], double sig, int pend, double eta_prev, const Policies& pol) {
+    if (pend) st_hint(V.ysum + i, r.ys + eta_prev * r.y, pol.first);
     const double v = r.y + sig * (r.q - kx[0]);
     const double yn = (r.isg && v < 0.0) ? 0.0 : v;
-    ynext[i] = yn;
+    st_hint(ynext + i, yn, pol.last);                       // gathered by the next k_primal: keep it in L2
     return yn - r.y;
 }
 
 __global__ void __launch_bounds__(kAttemptThreads, kCtasPerSm) k_dual(Sell K, Vecs V, Ctrl* ctl) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    DualPipe& P = *reinterpret_cast<DualPipe*>(smem_raw);
+    DualSmem& P = *reinterpret_cast<DualSmem*>(smem_raw);
     if (ld_flag(&ctl->done)) return;
     const int cur = ctl->cur, pend = ctl->pending;
     const double eta_prev = ctl->eta_prev, sig = ctl->eta * ctl->omega;
@@ -273,22 +292,11 @@ __global__ void __launch_bounds__(kAttemptThreads, kCtasPerSm) k_dual(Sell K, Ve
     double* __restrict__ ynext = V.y[cur ^ 1];
     const double2* __restrict__ xg = V.xg;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    pipe_init(P);
     dd acc[2] = {dd{0.0, 0.0}, dd{0.0, 0.0}};
-    auto gather = [&](int c, double (&o)[2]) { const double2 t = __ldg(xg + c); o[0] = t.x; o[1] = t.y; };
+    const Policies pol{policy_evict_first(), policy_evict_last()};
 
-    if (warp == kCons) {                                   // ---- producer
-        producer_loop(K, P, lane, [&](auto& S, long long row0, int rows, uint64_t* bar) -> uint32_t {
-            const uint32_t b = 8u * (uint32_t)rows;
-            if (bar) {
-                tma_load(S.vec[0], ycur + row0, b, bar);
-                tma_load(S.vec[1], V.q + row0, b, bar);
-                if (pend) tma_load(S.vec[2], V.ysum + row0, b, bar);
-                tma_load(S.bvec, V.isG + row0, (uint32_t)rows, bar);
-            }
-            return (pend ? 3u : 2u) * b + (uint32_t)rows;
-        });
-    } else if (warp == kCons + 1) {                        // ---- long rows
+    if (warp == kAttWarps) {                               // ---- long rows
+        auto gather = [&](int c, double (&o)[2]) { const double2 t = __ldg(xg + c); o[0] = t.x; o[1] = t.y; };
         for (int r = blockIdx.x; r < K.nlong; r += gridDim.x) {
             const long long i = K.nshort + r;
             DualRow dr{0.0, 0.0, 0.0, 0};
@@ -296,35 +304,39 @@ __global__ void __launch_bounds__(kAttemptThreads, kCtasPerSm) k_dual(Sell K, Ve
             double kx[2] = {0.0, 0.0};
             long_row<2>(K, r, lane, kx, gather);
             if (lane == 0) {
-                const double dy = dual_update(V, ynext, i, dr, kx, sig, pend, eta_prev);
+                const double dy = dual_update(V, ynext, i, dr, kx, sig, pend, eta_prev, pol);
                 acc[0] = dd_add_d(acc[0], dy * dy); acc[1] = dd_add_d(acc[1], dy * kx[1]);
             }
         }
-    } else {                                               // ---- consumers
-        int t = blockIdx.x;
-        for (int it = 0; t < K.ntiles; ++it, t += gridDim.x) {
-            const int s = it % kStages;
-            mbar_wait(&P.full[s], (uint32_t)(it / kStages) & 1u);
-            auto& S = P.st[s];
-            if (warp < S.hdr.nslices) {
-                const long long i = 32LL * (S.hdr.first_slice + warp) + lane;
-                const int r = warp * 32 + lane;
-                const int off = S.hdr.woff[warp], width = (S.hdr.woff[warp + 1] - off) >> 5;
-                DualRow dr{S.vec[0][r], S.vec[1][r], pend ? S.vec[2][r] : 0.0, (int)S.bvec[r]};
-                double kx[2] = {0.0, 0.0};
-                if (S.hdr.staged) slice_row<2>(S.col + off, S.val + off, width, lane, kx, gather);
-                else slice_row<2>(K.col + S.hdr.span_base + off, (const double*)K.val + S.hdr.span_base + off, width, lane, kx, gather);
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&P.empty[s]);
-                if (i < K.nshort) {
-                    const double dy = dual_update(V, ynext, i, dr, kx, sig, pend, eta_prev);
-                    acc[0] = dd_add_d(acc[0], dy * dy); acc[1] = dd_add_d(acc[1], dy * kx[1]);
-                }
-            } else {
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&P.empty[s]);
-            }
+    } else {                                               // ---- consumer warps
+        double kx[2] = {0.0, 0.0};
+        // this lane's share of a slice's vector segments: piece k covers vector v = 2k + lane/16, doubles off, off+1
+        const double* vsrc[2]; int voff[2]; bool vok[2];
+#pragma unroll
+        for (int k = 0; k < 2; ++k) {
+            const int v = 2 * k + (lane >> 4), off = (lane & 15) * 2;
+            vsrc[k] = (v == 0 ? ycur : v == 1 ? V.q : V.ysum) + off;
+            voff[k] = v * 32 + off; vok[k] = v < 2 || (v == 2 && pend);
         }
+        warp_pipeline(K, P.w[warp], (int)blockIdx.x * kAttWarps + warp, lane, xg, pol.first,
+            [&](auto& D, int row0) {                       // y, q (, ysum): 16 pieces each; isG: 2 pieces
+#pragma unroll
+                for (int k = 0; k < 2; ++k)
+                    if (vok[k]) cp_stream16(&D.vec[0][0] + voff[k], vsrc[k] + row0, pol.first);
+                if (lane == 16 || lane == 17) cp_stream16(&D.bvec[(lane - 16) * 16], V.isG + row0 + (lane - 16) * 16, pol.first);
+            },
+            [&](auto& D, int info, int row0) {
+                if (info & 16) { kx[0] = 0.0; kx[1] = 0.0; }
+                step_sum<2>(D.val, D.gv, info & 7, lane, kx);
+                if (info & 32) {
+                    const long long i = (long long)row0 + lane;
+                    if (i < K.nshort) {
+                        const DualRow dr{D.vec[0][lane], D.vec[1][lane], pend ? D.vec[2][lane] : 0.0, (int)D.bvec[lane]};
+                        const double dy = dual_update(V, ynext, i, dr, kx, sig, pend, eta_prev, pol);
+                        acc[0] = dd_add_d(acc[0], dy * dy); acc[1] = dd_add_d(acc[1], dy * kx[1]);
+                    }
+                }
+            });
     }
     block_sum_dd<2>(acc, P.red);
     if (threadIdx.x == 0) { V.partB[blockIdx.x] = acc[0]; V.partB[V.gridPB + blockIdx.x] = acc[1]; }

@@ -14,9 +14,24 @@
 #include <string>
 #include <vector>
 #include <algorithm>
+#include <queue>
+#include <functional>
+#include <utility>
 #include <cmath>
 
 namespace ucpdhg {
+
+// One step of the warp-private pipelines of the persistent attempt kernels (uc_attempt.cuh): a chunk of at
+// most kChunkT entries per row of one slice.  A slice wider than kChunkT is a run of consecutive steps of
+// the same warp, the row sums carried in registers from one to the next.  16 bytes.
+constexpr int kChunkT = 4;
+struct StepDesc {
+    long long ebase;   // first stored entry of the chunk in the sliced-ELL arrays
+    int row0;          // first row of the slice
+    int info;          // bits 0-2: entries per row in this chunk (0 = padding step: nothing to do); bit 4: first chunk
+                       // of its slice; bit 5: last chunk of its slice (the update is applied)
+};
+static_assert(sizeof(StepDesc) == 16, "StepDesc layout");
 
 struct HostSell {
     int64_t nrows = 0, nshort = 0, nlong = 0, nslices = 0;
@@ -28,21 +43,52 @@ struct HostSell {
     std::vector<int32_t> lcol;
     std::vector<double> lval;
     std::vector<int64_t> lsrc;
-    std::vector<int32_t> tile_ptr;    // [ntiles+1] first slice of each tile of the persistent attempt kernels
+    std::vector<StepDesc> steps;      // [steps_per_warp][sched_warps] schedule of the persistent attempt kernels
+    int64_t steps_per_warp = 0, sched_warps = 0;
 };
 
-// Tiles of the persistent attempt kernels: consecutive slices, at most `max_slices` of them (one per
-// consumer warp) and at most `cap` stored entries in total (what one shared-memory stage holds).  A
-// single slice wider than `cap` forms a tile of its own (read straight from global memory).
-inline void build_tiles(HostSell& S, int max_slices, int64_t cap) {
-    S.tile_ptr.clear();
-    S.tile_ptr.push_back(0);
-    int64_t s = 0;
-    while (s < S.nslices) {
-        int64_t e = s + 1;
-        while (e < S.nslices && e - s < max_slices && S.slice_ptr[(size_t)e + 1] - S.slice_ptr[(size_t)s] <= cap) ++e;
-        S.tile_ptr.push_back((int32_t)e);
-        s = e;
+// Static schedule of the persistent attempt kernels for `warps` consumer warps in total.  Slices are taken in
+// ascending order and each goes to the warp with the fewest steps so far (ties: lowest warp), so that the
+// warps' step counts differ by at most one slice's worth while, at any moment, all warps work on neighbouring
+// slices (DRAM pages and L2 lines are shared).  A warp takes its slices in ascending order, each as
+// ceil(width / kChunkT) steps.  Stored step-major, steps[j * warps + w], padded with empty steps to the
+// longest warp, so that step j of all warps is one coalesced read.  The assignment is fixed at create time:
+// solves are reproducible bit for bit.
+inline void build_schedule(HostSell& S, int64_t warps) {
+    if (warps < 1) warps = 1;
+    S.sched_warps = warps;
+    std::vector<int32_t> owner((size_t)S.nslices);
+    std::vector<int64_t> count((size_t)warps, 0);
+    {
+        typedef std::pair<int64_t, int64_t> Load;                    // (steps so far, warp)
+        std::priority_queue<Load, std::vector<Load>, std::greater<Load>> heap;
+        for (int64_t w = 0; w < warps; ++w) heap.push(Load(0, w));
+        for (int64_t s = 0; s < S.nslices; ++s) {
+            const int64_t wd = (S.slice_ptr[(size_t)s + 1] - S.slice_ptr[(size_t)s]) / 32;
+            Load l = heap.top(); heap.pop();
+            owner[(size_t)s] = (int32_t)l.second;
+            l.first += std::max<int64_t>(1, (wd + kChunkT - 1) / kChunkT);
+            count[(size_t)l.second] = l.first;
+            heap.push(l);
+        }
+    }
+    int64_t J = 0;
+    for (int64_t c : count) J = std::max(J, c);
+    S.steps_per_warp = J;
+    S.steps.assign((size_t)(J * warps), StepDesc{0, 0, 0});
+    std::fill(count.begin(), count.end(), 0);
+    for (int64_t s = 0; s < S.nslices; ++s) {
+        const int64_t wd = (S.slice_ptr[(size_t)s + 1] - S.slice_ptr[(size_t)s]) / 32;
+        const int64_t nch = std::max<int64_t>(1, (wd + kChunkT - 1) / kChunkT);
+        const int64_t w = owner[(size_t)s];
+        for (int64_t c = 0; c < nch; ++c) {
+            StepDesc d;
+            d.ebase = S.slice_ptr[(size_t)s] + 32 * kChunkT * c;
+            d.row0 = (int)(32 * s);
+            const int64_t nt = std::min<int64_t>(kChunkT, wd - kChunkT * c);
+            d.info = (int)std::max<int64_t>(nt, 0) | (c == 0 ? 16 : 0) | (c == nch - 1 ? 32 : 0);
+            S.steps[(size_t)(count[(size_t)w]++ * warps + w)] = d;
+        }
     }
 }
 

@@ -18,6 +18,7 @@
 #include <math.h>
 #include "../../include/uc_pdhg.h"
 #include "uc_dd.cuh"
+#include "uc_format.hpp"
 
 namespace ucpdhg {
 
@@ -65,8 +66,8 @@ struct Sell {
     int nlong;
     int nlblk;             // blocks covering the long tail = ceil(nlong / kWarps); they come FIRST in the grid
     int grid;              // nlblk + nblk, at least 1
-    const int* tile_ptr;   // [ntiles+1] first slice of each tile of the persistent attempt kernels (uc_attempt.cuh)
-    int ntiles;
+    const StepDesc* steps;  // [steps_per_warp][sched_warps] schedule of the persistent attempt kernels (uc_attempt.cuh)
+    int steps_per_warp, sched_warps;
 };
 
 struct Vecs {

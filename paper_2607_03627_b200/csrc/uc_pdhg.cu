@@ -117,8 +117,8 @@ Sell upload_sell(uc_lp* lp, const HostSell& H) {
     S.nlblk = cdiv(H.nlong, kWarps);
     S.grid = S.nlblk + S.nblk;
     if (S.grid < 1) S.grid = 1;
-    S.tile_ptr = lp->upload(H.tile_ptr);
-    S.ntiles = (int)H.tile_ptr.size() - 1;
+    S.steps = lp->upload(H.steps);
+    S.steps_per_warp = (int)H.steps_per_warp; S.sched_warps = (int)H.sched_warps;
     return S;
 }
 
@@ -172,8 +172,8 @@ void ensure_powtab(uc_lp* lp, long long limit) {
 }
 
 void launch_attempt(uc_lp* lp, cudaStream_t st) {
-    k_primal<<<lp->V.gridPA, kAttemptThreads, sizeof(PrimalPipe), st>>>(lp->KT, lp->V, lp->ctl);
-    k_dual<<<lp->V.gridPB, kAttemptThreads, sizeof(DualPipe), st>>>(lp->K, lp->V, lp->ctl);
+    k_primal<<<lp->V.gridPA, kAttemptThreads, sizeof(PrimalSmem), st>>>(lp->KT, lp->V, lp->ctl);
+    k_dual<<<lp->V.gridPB, kAttemptThreads, sizeof(DualSmem), st>>>(lp->K, lp->V, lp->ctl);
 }
 void launch_kkt(uc_lp* lp, cudaStream_t st, int mode) {
     k_check_dual<<<lp->KT.grid, kBlock, 0, st>>>(lp->KT, lp->V, lp->ctl);
@@ -239,9 +239,9 @@ void destroy_impl(uc_lp* lp) {
 
 int64_t bytes_per_attempt(const uc_lp* lp) {
     // what one attempt streams in THIS layout: matrix slots (12 B each, padding included),
-    // slice pointers, and per variable 8 (x) + 24 (c,l,u) + 16 (xsum r/w) + 8 (x') + 16 ({xbar,dx}) + 16
+    // step descriptors (16 B per scheduled step, padding steps included), and per variable 8 (x) + 24 (c,l,u) + 16 (xsum r/w) + 8 (x') + 16 ({xbar,dx}) + 16
     // (gather of the pair) = 88 B, per row 8 (y) + 8 (q) + 1 (sense) + 16 (ysum r/w) + 8 (y') + 8 (gather) = 49 B
-    return 12 * (lp->k_slots + lp->kt_slots + lp->k_long_nnz + lp->kt_long_nnz) + 8 * ((int64_t)lp->K.nslices + lp->KT.nslices) +
+    return 12 * (lp->k_slots + lp->kt_slots + lp->k_long_nnz + lp->kt_long_nnz) + 16 * ((int64_t)lp->K.steps_per_warp * lp->K.sched_warps + (int64_t)lp->KT.steps_per_warp * lp->KT.sched_warps) +
            88 * lp->n + 49 * lp->m;
 }
 
@@ -251,6 +251,7 @@ int64_t bytes_per_attempt(const uc_lp* lp) {
 extern "C" {
 
 const char* uc_last_error(void) { return g_err.c_str(); }
+
 
 double uc_host_log_rounded(double a) { return log_rounded(a); }
 double uc_host_exp_rounded(double x) { return exp_rounded(x); }
@@ -304,8 +305,17 @@ int uc_lp_create(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, cons
         // A0 / A1: layouts (host), upload
         HostProblem P;
         build_problem(m, n, nnz, row_ptr, col_idx, val, opt.sell_window, opt.long_row_threshold, opt.keep_source_map != 0, P);
-        build_tiles(P.K, kCons, kCap);
-        build_tiles(P.KT, kCons, kCap);
+        int gridPA = 1, gridPB = 1;
+        {   // persistent grids of the attempt kernels: kCtasPerSm CTAs per SM, never more CTAs than work; the static
+            // schedule gives slice s to consumer warp s % (grid * kAttWarps)
+            int sms = 0;
+            CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+            const int cap = kCtasPerSm * std::max(sms, 1);
+            gridPA = (int)std::max<int64_t>(1, std::min<int64_t>(cap, std::max<int64_t>((P.KT.nslices + kAttWarps - 1) / kAttWarps, P.KT.nlong)));
+            gridPB = (int)std::max<int64_t>(1, std::min<int64_t>(cap, std::max<int64_t>((P.K.nslices + kAttWarps - 1) / kAttWarps, P.K.nlong)));
+            build_schedule(P.KT, (int64_t)gridPA * kAttWarps);
+            build_schedule(P.K, (int64_t)gridPB * kAttWarps);
+        }
         lp->K = upload_sell(lp, P.K);
         lp->KT = upload_sell(lp, P.KT);
         lp->k_slots = (int64_t)P.K.col.size(); lp->kt_slots = (int64_t)P.KT.col.size();
@@ -326,15 +336,9 @@ int uc_lp_create(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, cons
         lp->Dr = lp->dalloc<double>((size_t)m); lp->Dc = lp->dalloc<double>((size_t)n);
         V.c = lp->cs; V.l = lp->ls; V.u = lp->us; V.q = lp->qs; V.isG = lp->isG; V.Dr = lp->Dr; V.Dc = lp->Dc;
         V.gridA = lp->KT.grid; V.gridB = lp->K.grid; V.gridR = std::max(1, cdiv(n + m, kBlock));
-        {   // persistent grids of the attempt kernels: kCtasPerSm CTAs per SM, never more CTAs than work items
-            int sms = 0;
-            CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-            const int cap = kCtasPerSm * std::max(sms, 1);
-            V.gridPA = std::max(1, std::min(cap, std::max(lp->KT.ntiles, lp->KT.nlong)));
-            V.gridPB = std::max(1, std::min(cap, std::max(lp->K.ntiles, lp->K.nlong)));
-            CK(cudaFuncSetAttribute(k_primal, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(PrimalPipe)));
-            CK(cudaFuncSetAttribute(k_dual, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(DualPipe)));
-        }
+        V.gridPA = gridPA; V.gridPB = gridPB;
+        CK(cudaFuncSetAttribute(k_primal, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(PrimalSmem)));
+        CK(cudaFuncSetAttribute(k_dual, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(DualSmem)));
         V.partA = lp->dalloc<dd>((size_t)V.gridPA);
         V.partB = lp->dalloc<dd>((size_t)2 * V.gridPB);
         V.partD = lp->dalloc<dd>((size_t)8 * V.gridA);
@@ -576,9 +580,9 @@ int uc_pdhg_time_kernels(uc_lp* lp, void* stream, int32_t attempts, double* prim
         for (auto& e : ev) CK(cudaEventCreate(&e));
         CK(cudaEventRecord(ev[0], st));
         for (int i = 0; i < attempts; ++i) {
-            k_primal<<<lp->V.gridPA, kAttemptThreads, sizeof(PrimalPipe), st>>>(lp->KT, lp->V, lp->ctl);
+            k_primal<<<lp->V.gridPA, kAttemptThreads, sizeof(PrimalSmem), st>>>(lp->KT, lp->V, lp->ctl);
             CK(cudaEventRecord(ev[(size_t)2 * i + 1], st));
-            k_dual<<<lp->V.gridPB, kAttemptThreads, sizeof(DualPipe), st>>>(lp->K, lp->V, lp->ctl);
+            k_dual<<<lp->V.gridPB, kAttemptThreads, sizeof(DualSmem), st>>>(lp->K, lp->V, lp->ctl);
             CK(cudaEventRecord(ev[(size_t)2 * i + 2], st));
         }
         CK(cudaStreamSynchronize(st));
