@@ -125,9 +125,12 @@ static_assert(kCtasPerSm * (sizeof(PrimalSmem) + 1024) <= 228 * 1024 && kCtasPer
 // The schedule is read 32 steps at a time (lane l holds step 32 b + l of the warp; the next batch is loaded
 // one batch ahead) and a step's descriptor travels from A to B to C through two small register queues, so
 // only the A cursor ever touches it.
-template <class Ring, class GT, class FV, class FC>
-__device__ __forceinline__ void warp_pipeline(const Sell& A, Ring& R, int gw, int lane, const GT* __restrict__ gsrc,
-                                              uint64_t pol_first, FV issue_vecs, FC compute) {
+// dep_ready() is called once, just before the first B stage: everything before it (schedule loads, the first
+// index copies) touches only data that no kernel writes, so it overlaps the tail of the previous kernel
+// (programmatic dependent launch); it returns false if the solve is already over.
+template <class Ring, class GT, class FD, class FV, class FC>
+__device__ __forceinline__ bool warp_pipeline(const Sell& A, Ring& R, int gw, int lane, const GT* const& gsrc,
+                                              uint64_t pol_first, FD dep_ready, FV issue_vecs, FC compute) {
     const int J = A.steps_per_warp;
     const long long GW = A.sched_warps;
     auto load_desc = [&](int k) -> int4 {
@@ -143,6 +146,7 @@ __device__ __forceinline__ void warp_pipeline(const Sell& A, Ring& R, int gw, in
     // ring slots of steps ka (index ring), kb (index ring: kb = ka - (kRingA - 1)), kb (data ring: kb = -kRingB at the start), j
     int sa = 0, sbA = 1 % kRingA, sb = 0, sc = 0;
     for (int j = -kDA; j < J; ++j) {
+        if (j == -kDB && !dep_ready()) { cp_wait<0>(); return false; }
         // ---- A: column indices of step ka = j + kDA
         const int ka = j + kDA;
         if (ka >= 32 && (ka & 31) == 0) { dcur = dnxt; dnxt = load_desc(ka + 32 + lane); }
@@ -184,7 +188,14 @@ __device__ __forceinline__ void warp_pipeline(const Sell& A, Ring& R, int gw, in
         if (j >= 0) sc = (sc + 1 == kRingB) ? 0 : sc + 1;
     }
     cp_wait<0>();
+    return true;
 }
+
+// Programmatic dependent launch (PDL): the next kernel in the stream may start its prologue as soon as every
+// CTA of this one has passed grid_launch_dependents(); grid_dependency_wait() returns once the previous kernel
+// has completed and its writes are visible.
+__device__ __forceinline__ void grid_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void grid_dependency_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
 // Row sum contribution of one step: entries t*32+lane of the slot, t = 0..nt-1, left to right.
 template <int NV, class GT>
@@ -219,17 +230,32 @@ __device__ __forceinline__ double primal_update(const Vecs& V, double* __restric
 __global__ void __launch_bounds__(kAttemptThreads, kCtasPerSm) k_primal(Sell KT, Vecs V, Ctrl* ctl) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     PrimalSmem& P = *reinterpret_cast<PrimalSmem*>(smem_raw);
-    if (ld_flag(&ctl->done)) return;
-    const int cur = ctl->cur, pend = ctl->pending;
-    const double eta_prev = ctl->eta_prev, tau = ctl->eta / ctl->omega;
-    const double* __restrict__ xcur = V.x[cur];
-    const double* __restrict__ ycur = V.y[cur];
-    double* __restrict__ xnext = V.x[cur ^ 1];
+    grid_launch_dependents();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     dd acc[1] = {dd{0.0, 0.0}};
     const Policies pol{policy_evict_first(), policy_evict_last()};
+    // everything below is set by dep_ready(), i.e. read after the previous kernel has completed
+    int pend = 0; double eta_prev = 0.0, tau = 0.0;
+    const double* xcur = nullptr; const double* ycur = nullptr; double* xnext = nullptr;
+    const double* vsrc[3]; int voff[3]; bool vok[3];   // this lane's share of a slice's vector segments: piece k covers
+                                                       // vector v = 2k + lane/16, doubles off, off+1
+    auto dep_ready = [&]() -> bool {
+        grid_dependency_wait();
+        if (ld_flag(&ctl->done)) return false;
+        const int cur = ctl->cur;
+        pend = ctl->pending; eta_prev = ctl->eta_prev; tau = ctl->eta / ctl->omega;
+        xcur = V.x[cur]; ycur = V.y[cur]; xnext = V.x[cur ^ 1];
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const int v = 2 * k + (lane >> 4), off = (lane & 15) * 2;
+            vsrc[k] = (v == 0 ? xcur : v == 1 ? V.c : v == 2 ? V.l : v == 3 ? V.u : V.xsum) + off;
+            voff[k] = v * 32 + off; vok[k] = v < 4 || (v == 4 && pend);
+        }
+        return true;
+    };
 
     if (warp == kAttWarps) {                               // ---- long rows, one per pass
+        if (!dep_ready()) return;
         for (int r = blockIdx.x; r < KT.nlong; r += gridDim.x) {
             const long long j = KT.nshort + r;
             PrimalRow pr{0.0, 0.0, 0.0, 0.0, 0.0};
@@ -240,15 +266,7 @@ __global__ void __launch_bounds__(kAttemptThreads, kCtasPerSm) k_primal(Sell KT,
         }
     } else {                                               // ---- consumer warps
         double g[1] = {0.0};
-        // this lane's share of a slice's vector segments: piece k covers vector v = 2k + lane/16, doubles off, off+1
-        const double* vsrc[3]; int voff[3]; bool vok[3];
-#pragma unroll
-        for (int k = 0; k < 3; ++k) {
-            const int v = 2 * k + (lane >> 4), off = (lane & 15) * 2;
-            vsrc[k] = (v == 0 ? xcur : v == 1 ? V.c : v == 2 ? V.l : v == 3 ? V.u : V.xsum) + off;
-            voff[k] = v * 32 + off; vok[k] = v < 4 || (v == 4 && pend);
-        }
-        warp_pipeline(KT, P.w[warp], (int)blockIdx.x * kAttWarps + warp, lane, ycur, pol.first,
+        const bool live = warp_pipeline(KT, P.w[warp], (int)blockIdx.x * kAttWarps + warp, lane, ycur, pol.first, dep_ready,
             [&](auto& D, int row0) {                       // x, c, l, u (, xsum): 16 pieces of 16 bytes each
 #pragma unroll
                 for (int k = 0; k < 3; ++k)
@@ -265,6 +283,7 @@ __global__ void __launch_bounds__(kAttemptThreads, kCtasPerSm) k_primal(Sell KT,
                     }
                 }
             });
+        if (!live) return;
     }
     block_sum_dd<1>(acc, P.red);
     if (threadIdx.x == 0) V.partA[blockIdx.x] = acc[0];
@@ -285,17 +304,31 @@ __device__ __forceinline__ double dual_update(const Vecs& V, double* __restrict_
 __global__ void __launch_bounds__(kAttemptThreads, kCtasPerSm) k_dual(Sell K, Vecs V, Ctrl* ctl) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     DualSmem& P = *reinterpret_cast<DualSmem*>(smem_raw);
-    if (ld_flag(&ctl->done)) return;
-    const int cur = ctl->cur, pend = ctl->pending;
-    const double eta_prev = ctl->eta_prev, sig = ctl->eta * ctl->omega;
-    const double* __restrict__ ycur = V.y[cur];
-    double* __restrict__ ynext = V.y[cur ^ 1];
-    const double2* __restrict__ xg = V.xg;
+    grid_launch_dependents();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     dd acc[2] = {dd{0.0, 0.0}, dd{0.0, 0.0}};
     const Policies pol{policy_evict_first(), policy_evict_last()};
+    const double2* xg = V.xg;
+    // everything below is set by dep_ready(), i.e. read after the previous kernel has completed
+    int cur = 0, pend = 0; double eta_prev = 0.0, sig = 0.0;
+    const double* ycur = nullptr; double* ynext = nullptr;
+    const double* vsrc[2]; int voff[2]; bool vok[2];   // this lane's share of a slice's vector segments
+    auto dep_ready = [&]() -> bool {
+        grid_dependency_wait();
+        if (ld_flag(&ctl->done)) return false;
+        cur = ctl->cur; pend = ctl->pending; eta_prev = ctl->eta_prev; sig = ctl->eta * ctl->omega;
+        ycur = V.y[cur]; ynext = V.y[cur ^ 1];
+#pragma unroll
+        for (int k = 0; k < 2; ++k) {
+            const int v = 2 * k + (lane >> 4), off = (lane & 15) * 2;
+            vsrc[k] = (v == 0 ? ycur : v == 1 ? V.q : V.ysum) + off;
+            voff[k] = v * 32 + off; vok[k] = v < 2 || (v == 2 && pend);
+        }
+        return true;
+    };
 
     if (warp == kAttWarps) {                               // ---- long rows
+        if (!dep_ready()) return;
         auto gather = [&](int c, double (&o)[2]) { const double2 t = __ldg(xg + c); o[0] = t.x; o[1] = t.y; };
         for (int r = blockIdx.x; r < K.nlong; r += gridDim.x) {
             const long long i = K.nshort + r;
@@ -310,15 +343,7 @@ __global__ void __launch_bounds__(kAttemptThreads, kCtasPerSm) k_dual(Sell K, Ve
         }
     } else {                                               // ---- consumer warps
         double kx[2] = {0.0, 0.0};
-        // this lane's share of a slice's vector segments: piece k covers vector v = 2k + lane/16, doubles off, off+1
-        const double* vsrc[2]; int voff[2]; bool vok[2];
-#pragma unroll
-        for (int k = 0; k < 2; ++k) {
-            const int v = 2 * k + (lane >> 4), off = (lane & 15) * 2;
-            vsrc[k] = (v == 0 ? ycur : v == 1 ? V.q : V.ysum) + off;
-            voff[k] = v * 32 + off; vok[k] = v < 2 || (v == 2 && pend);
-        }
-        warp_pipeline(K, P.w[warp], (int)blockIdx.x * kAttWarps + warp, lane, xg, pol.first,
+        const bool live = warp_pipeline(K, P.w[warp], (int)blockIdx.x * kAttWarps + warp, lane, xg, pol.first, dep_ready,
             [&](auto& D, int row0) {                       // y, q (, ysum): 16 pieces each; isG: 2 pieces
 #pragma unroll
                 for (int k = 0; k < 2; ++k)
@@ -337,6 +362,7 @@ __global__ void __launch_bounds__(kAttemptThreads, kCtasPerSm) k_dual(Sell K, Ve
                     }
                 }
             });
+        if (!live) return;
     }
     block_sum_dd<2>(acc, P.red);
     if (threadIdx.x == 0) { V.partB[blockIdx.x] = acc[0]; V.partB[V.gridPB + blockIdx.x] = acc[1]; }
@@ -347,9 +373,13 @@ __global__ void __launch_bounds__(kAttemptThreads, kCtasPerSm) k_dual(Sell K, Ve
     }
     __syncthreads();
     if (!P.is_last) return;
-    const dd sdx = final_sum(V.partA, V.gridPA, P.red);
-    const dd sdy = final_sum(V.partB, V.gridPB, P.red);
-    const dd sin_ = final_sum(V.partB + V.gridPB, V.gridPB, P.red);
+    dd sdx, sdy, sin_;
+    {
+        dd a[1], b[2];
+        final_sums<1>(V.partA, 0, V.gridPA, a, P.red);
+        final_sums<2>(V.partB, V.gridPB, V.gridPB, b, P.red);
+        sdx = a[0]; sdy = b[0]; sin_ = b[1];
+    }
     if (threadIdx.x != 0) return;
     ctl->ticket_b = 0;
     const double dx2 = dd_round(sdx), dy2 = dd_round(sdy), inter = fabs(dd_round(sin_));

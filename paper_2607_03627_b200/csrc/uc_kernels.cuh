@@ -119,8 +119,9 @@ __device__ __forceinline__ dd warp_sum_dd(dd v) {
     return v;
 }
 
-// block-wide double-double sums of NV values (each thread contributes one double per value);
-// result valid in thread 0.  red: NV * 32 dd of shared memory.
+// block-wide double-double sums of NV values (each thread contributes one double-double per value);
+// result valid in thread 0.  red: NV * 32 dd of shared memory.  Two stages, both warp-parallel: every warp
+// reduces its own NV values by shuffles, then warp q (mod #warps) reduces the per-warp results of value q.
 template <int NV>
 __device__ __forceinline__ void block_sum_dd(dd (&v)[NV], dd* red) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
@@ -130,13 +131,15 @@ __device__ __forceinline__ void block_sum_dd(dd (&v)[NV], dd* red) {
         if (lane == 0) red[q * 32 + warp] = v[q];
     }
     __syncthreads();
+    for (int q = warp; q < NV; q += nw) {
+        dd t = lane < nw ? red[q * 32 + lane] : dd{0.0, 0.0};
+        t = warp_sum_dd(t);
+        if (lane == 0) red[q * 32] = t;
+    }
+    __syncthreads();
     if (threadIdx.x == 0) {
 #pragma unroll
-        for (int q = 0; q < NV; ++q) {
-            dd s = red[q * 32];
-            for (int w = 1; w < nw; ++w) s = dd_add(s, red[q * 32 + w]);
-            v[q] = s;
-        }
+        for (int q = 0; q < NV; ++q) v[q] = red[q * 32];
     }
     __syncthreads();
 }
@@ -153,14 +156,24 @@ __device__ __forceinline__ bool last_block_done(unsigned int* ticket) {
     return is_last != 0;
 }
 
-// double-double sum of a partial array by one block; result valid in thread 0
-__device__ __forceinline__ dd final_sum(const dd* part, int count, dd* red) {
-    dd v[1] = {dd{0.0, 0.0}};
+// double-double sums of NV partial arrays (part + q * stride, `count` entries each) by one block, in one pass;
+// results valid in thread 0
+template <int NV>
+__device__ __forceinline__ void final_sums(const dd* part, long long stride, int count, dd (&v)[NV], dd* red) {
+#pragma unroll
+    for (int q = 0; q < NV; ++q) v[q] = dd{0.0, 0.0};
     for (int i = threadIdx.x; i < count; i += blockDim.x) {
-        dd t; t.hi = __ldcg(&part[i].hi); t.lo = __ldcg(&part[i].lo);
-        v[0] = dd_add(v[0], t);
+#pragma unroll
+        for (int q = 0; q < NV; ++q) {
+            dd t; t.hi = __ldcg(&part[q * stride + i].hi); t.lo = __ldcg(&part[q * stride + i].lo);
+            v[q] = dd_add(v[q], t);
+        }
     }
-    block_sum_dd<1>(v, red);
+    block_sum_dd<NV>(v, red);
+}
+__device__ __forceinline__ dd final_sum(const dd* part, int count, dd* red) {
+    dd v[1];
+    final_sums<1>(part, 0, count, v, red);
     return v[0];
 }
 
@@ -387,12 +400,19 @@ enum { kModeInit = 0,    // z^0: store the KKT components of the restart point (
 
 // A11 end + A12 decision + A13: single block.
 __global__ void __launch_bounds__(kFinalBlock) k_check_finalize(Vecs V, Ctrl* ctl, int mode) {
-    __shared__ dd red[32];
-    __shared__ dd T[14];
+    __shared__ dd red[8 * 32];
     if (ld_flag(&ctl->done)) return;
-    for (int q = 0; q < 8; ++q) { dd s = final_sum(V.partD + (long long)q * V.gridA, V.gridA, red); if (threadIdx.x == 0) T[q] = s; }
-    for (int q = 0; q < 6; ++q) { dd s = final_sum(V.partP + (long long)q * V.gridB, V.gridB, red); if (threadIdx.x == 0) T[8 + q] = s; }
-    if (threadIdx.x != 0) return;
+    dd T[14];
+    {
+        dd a[8], b[6];
+        final_sums<8>(V.partD, V.gridA, V.gridA, a, red);
+        final_sums<6>(V.partP, V.gridB, V.gridB, b, red);
+        if (threadIdx.x != 0) return;
+#pragma unroll
+        for (int q = 0; q < 8; ++q) T[q] = a[q];
+#pragma unroll
+        for (int q = 0; q < 6; ++q) T[8 + q] = b[q];
+    }
     const bool have_avg = ctl->w > 0.0;
     KktT Tc, Ta;
     Tc.rd2_s = dd_round(T[0]); Tc.rd2_u = dd_round(T[1]); Tc.pobj = dd_round(T[2]);
@@ -470,12 +490,12 @@ __global__ void __launch_bounds__(kBlock) k_restart_vec(Vecs V, Ctrl* ctl) {
 }
 // A12 restart, scalars: primal weight (R11), w <- 0
 __global__ void __launch_bounds__(kFinalBlock) k_restart_finalize(Vecs V, Ctrl* ctl) {
-    __shared__ dd red[32];
+    __shared__ dd red[2 * 32];
     if (ld_flag(&ctl->done) || !ctl->restart_kind) return;
-    const dd sx = final_sum(V.partR, V.gridR, red);
-    const dd sy = final_sum(V.partR + V.gridR, V.gridR, red);
+    dd sxy[2];
+    final_sums<2>(V.partR, V.gridR, V.gridR, sxy, red);
     if (threadIdx.x != 0) return;
-    const double Dx = sqrt(dd_round(sx)), Dy = sqrt(dd_round(sy));
+    const double Dx = sqrt(dd_round(sxy[0])), Dy = sqrt(dd_round(sxy[1]));
     if (Dx > 1e-10 && Dy > 1e-10) {
         const double th = ctl->smoothing;
         ctl->omega = exp_rounded(th * log_rounded(Dy / Dx) + (1.0 - th) * log_rounded(ctl->omega));

@@ -171,10 +171,23 @@ void ensure_powtab(uc_lp* lp, long long limit) {
     lp->powtab_len = len;
 }
 
-void launch_attempt(uc_lp* lp, cudaStream_t st) {
-    k_primal<<<lp->V.gridPA, kAttemptThreads, sizeof(PrimalSmem), st>>>(lp->KT, lp->V, lp->ctl);
-    k_dual<<<lp->V.gridPB, kAttemptThreads, sizeof(DualSmem), st>>>(lp->K, lp->V, lp->ctl);
+// The two attempt kernels are launched with programmatic stream serialization (PDL): a kernel's prologue
+// (schedule loads, first index copies) overlaps the tail of the kernel before it; the kernel itself waits
+// (griddepcontrol.wait) before it reads anything a previous kernel wrote.  Captured into the graph as
+// programmatic dependency edges.
+template <class Kern>
+void launch_pdl(Kern kern, int grid, size_t smem, cudaStream_t st, const Sell& A, const Vecs& V, Ctrl* ctl) {
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3(kAttemptThreads); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    CK(cudaLaunchKernelEx(&cfg, kern, A, V, ctl));
 }
+void launch_primal(uc_lp* lp, cudaStream_t st) { launch_pdl(k_primal, lp->V.gridPA, sizeof(PrimalSmem), st, lp->KT, lp->V, lp->ctl); }
+void launch_dual(uc_lp* lp, cudaStream_t st) { launch_pdl(k_dual, lp->V.gridPB, sizeof(DualSmem), st, lp->K, lp->V, lp->ctl); }
+void launch_attempt(uc_lp* lp, cudaStream_t st) { launch_primal(lp, st); launch_dual(lp, st); }
 void launch_kkt(uc_lp* lp, cudaStream_t st, int mode) {
     k_check_dual<<<lp->KT.grid, kBlock, 0, st>>>(lp->KT, lp->V, lp->ctl);
     k_check_primal<<<lp->K.grid, kBlock, 0, st>>>(lp->K, lp->V, lp->ctl);
@@ -580,9 +593,9 @@ int uc_pdhg_time_kernels(uc_lp* lp, void* stream, int32_t attempts, double* prim
         for (auto& e : ev) CK(cudaEventCreate(&e));
         CK(cudaEventRecord(ev[0], st));
         for (int i = 0; i < attempts; ++i) {
-            k_primal<<<lp->V.gridPA, kAttemptThreads, sizeof(PrimalSmem), st>>>(lp->KT, lp->V, lp->ctl);
+            launch_primal(lp, st);
             CK(cudaEventRecord(ev[(size_t)2 * i + 1], st));
-            k_dual<<<lp->V.gridPB, kAttemptThreads, sizeof(DualSmem), st>>>(lp->K, lp->V, lp->ctl);
+            launch_dual(lp, st);
             CK(cudaEventRecord(ev[(size_t)2 * i + 2], st));
         }
         CK(cudaStreamSynchronize(st));
