@@ -118,6 +118,21 @@ using DualSmem = SmemT<3, true, double2>;     // y, q, ysum + isG ; gathers {xba
 static_assert(kCtasPerSm * (sizeof(PrimalSmem) + 1024) <= 228 * 1024 && kCtasPerSm * (sizeof(DualSmem) + 1024) <= 228 * 1024,
               "the CTAs of either attempt kernel must fit the shared memory of one SM");
 
+// Calls f(std::integral_constant<int, nt>) for nt = 1..kChunkT (nothing for nt = 0).  nt is warp-uniform, so
+// the branch does not diverge and each case is straight-line code without predicated-off instructions.
+template <int N> struct IntC { static constexpr int value = N; };
+template <class F>
+__device__ __forceinline__ void dispatch_nt(int nt, F f) {
+    static_assert(kChunkT == 4, "dispatch_nt covers 1..4");
+    switch (nt) {
+        case 1: f(IntC<1>{}); break;
+        case 2: f(IntC<2>{}); break;
+        case 3: f(IntC<3>{}); break;
+        case 4: f(IntC<4>{}); break;
+        default: break;
+    }
+}
+
 // ------------------------------------------------------------------------------------------ the pipeline
 // Runs the steps of consumer warp `gw` (of A.sched_warps) through the A / B / C pipeline described at the top.
 //   issue_vecs(slot, row0)    issues the cp.async copies of the 32-row vector segments of a slice
@@ -169,9 +184,13 @@ __device__ __forceinline__ bool warp_pipeline(const Sell& A, Ring& R, int gw, in
                 if (p < nt * 16) cp_stream16(&D.val[p * 2], A.val + eb + p * 2, pol_first);
             }
             if (info_b & 32) issue_vecs(D, row_b);
+            dispatch_nt(nt, [&](auto n) {
+                int c[decltype(n)::value];
 #pragma unroll
-            for (int t = 0; t < kChunkT; ++t)
-                if (t < nt) cp_gather(&D.gv[t * 32 + lane], gsrc + R.col[sbA][t * 32 + lane]);
+                for (int t = 0; t < decltype(n)::value; ++t) c[t] = R.col[sbA][t * 32 + lane];
+#pragma unroll
+                for (int t = 0; t < decltype(n)::value; ++t) cp_gather(&D.gv[t * 32 + lane], gsrc + c[t]);
+            });
         }
         cp_commit();
         // ---- C: step j
@@ -200,16 +219,17 @@ __device__ __forceinline__ void grid_dependency_wait() { asm volatile("griddepco
 // Row sum contribution of one step: entries t*32+lane of the slot, t = 0..nt-1, left to right.
 template <int NV, class GT>
 __device__ __forceinline__ void step_sum(const double* valp, const GT* gvp, int nt, int lane, double (&s)[NV]) {
-    double v[kChunkT]; GT g[kChunkT];
+    dispatch_nt(nt, [&](auto n) {
+        constexpr int N = decltype(n)::value;
+        double v[N]; GT g[N];
 #pragma unroll
-    for (int t = 0; t < kChunkT; ++t)
-        if (t < nt) { v[t] = valp[t * 32 + lane]; g[t] = gvp[t * 32 + lane]; }
+        for (int t = 0; t < N; ++t) { v[t] = valp[t * 32 + lane]; g[t] = gvp[t * 32 + lane]; }
 #pragma unroll
-    for (int t = 0; t < kChunkT; ++t)
-        if (t < nt) {
+        for (int t = 0; t < N; ++t) {
             if constexpr (NV == 1) s[0] = __dadd_rn(s[0], __dmul_rn(v[t], g[t]));
             else { s[0] = __dadd_rn(s[0], __dmul_rn(v[t], g[t].x)); s[1] = __dadd_rn(s[1], __dmul_rn(v[t], g[t].y)); }
         }
+    });
 }
 
 // ----------------------------------------------------------------- A5+A6 (+A10): primal kernel
