@@ -41,6 +41,11 @@ def algorithmic_bytes(m, n, nnz):
     return primal, dual
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the attempt kernels on config 3, from the one
+# `ncu --set full` capture summarised in profiles/r01c_summary.md (cold L2 per replay; bytes)
+NCU_TRAFFIC_CONFIG3 = {"k_primal": 185.75e6 + 12.06e6, "k_dual": 161.96e6 + 5.21e6, "source": "profiles/r01c_summary.md"}
+
+
 def load_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -226,7 +231,8 @@ def main():
         ach = dom[1] / (dom[2] * 1e-3) / 1e9
         att_ms = 1e3 * loop_s / (args.steps * A)
         roof = {"bound": "hbm", "kernel": dom[0], "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                "traffic": None, "peak_source": peak_src, "algorithmic_bytes_per_launch": dom[1], "kernel_ms": dom[2],
+                "traffic": NCU_TRAFFIC_CONFIG3[dom[0]] if args.config == 3 else None,
+                "traffic_source": NCU_TRAFFIC_CONFIG3["source"] if args.config == 3 else None, "peak_source": peak_src, "algorithmic_bytes_per_launch": dom[1], "kernel_ms": dom[2],
                 "other_kernel": {"k_primal_ms": primal_ms, "k_dual_ms": dual_ms, "k_primal_bytes": bp, "k_dual_bytes": bd},
                 "attempt": {"algorithmic_bytes": bp + bd, "ms_in_graph": att_ms, "GB/s": (bp + bd) / (att_ms * 1e-3) / 1e9,
                             "frac_of_peak": (bp + bd) / (att_ms * 1e-3) / 1e9 / peak,

@@ -14,7 +14,7 @@
 //   * a coalesced cp.async (LDGSTS.128) costs ~8 cycles and holds no register while in flight;
 //   * divergent gathers run at ~1000 gathers/us/SM from 4 issuing warps but ~1500 from 8 or more.
 // Hence: persistent CTAs (two per SM) of kAttWarps CONSUMER warps, every one of which runs its own
-// three-deep software pipeline on its own shared-memory rings, with NO block-level synchronisation inside
+// three-stage software pipeline on its own shared-memory rings, with NO block-level synchronisation inside
 // the loop.  The unit of work is a STEP (uc_format.hpp): up to kChunkT entries per row of one slice (32 rows,
 // one per lane).  For its step j a warp has, in flight at the same time,
 //     A(j + kDA): cp.async of the step's column indices                         -> index ring
@@ -24,8 +24,8 @@
 //                 {xbar, dx}, that e multiplies)                                -> data ring
 //     C(j):       everything read from shared memory: row sums left to right, update, coalesced stores.
 // One cp.async group is committed per step; cp.async.wait_group kDB + __syncwarp is the only wait.  A slice
-// wider than kChunkT is a run of consecutive steps whose row sums stay in registers.  The schedule (slice s ->
-// warp s % #warps, built at create time) is static, so results are reproducible bit for bit.  One extra warp
+// wider than kChunkT is a run of consecutive steps whose row sums stay in registers.  The schedule (each slice
+// to the least-loaded warp, built at create time) is static, so results are reproducible bit for bit.  One extra warp
 // per CTA takes the rows longer than the sliced-ELL threshold (the T reserve rows of the UC LP), one row at a
 // time, concurrently.
 // L2 policy: streamed-once data is loaded (cp.async.cg, L1 bypass) and stored evict_first; the gathered vectors
