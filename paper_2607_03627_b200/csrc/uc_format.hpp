@@ -17,6 +17,7 @@
 #include <queue>
 #include <functional>
 #include <utility>
+#include <thread>
 #include <cmath>
 
 namespace ucpdhg {
@@ -32,6 +33,22 @@ struct StepDesc {
                        // of its slice; bit 5: last chunk of its slice (the update is applied)
 };
 static_assert(sizeof(StepDesc) == 16, "StepDesc layout");
+
+// f(begin, end) over [0, n) on up to 8 host threads (uc_lp_create is a one-time cost, but it is inside the
+// end-to-end time: the layouts of a 6M-entry matrix take ~0.5 s on one core)
+template <class F>
+inline void parallel_ranges(int64_t n, int64_t grain, F f) {
+    unsigned hw = std::thread::hardware_concurrency();
+    int64_t nt = std::max<int64_t>(1, std::min<int64_t>(std::min<int64_t>(hw ? hw : 1, 8), n / std::max<int64_t>(grain, 1)));
+    if (nt <= 1) { f((int64_t)0, n); return; }
+    std::vector<std::thread> th;
+    const int64_t per = (n + nt - 1) / nt;
+    for (int64_t t = 0; t < nt; ++t) {
+        const int64_t b = t * per, e = std::min(n, b + per);
+        if (b < e) th.emplace_back([=] { f(b, e); });
+    }
+    for (auto& x : th) x.join();
+}
 
 struct HostSell {
     int64_t nrows = 0, nshort = 0, nlong = 0, nslices = 0;
@@ -129,26 +146,31 @@ inline void build_sell(int64_t nrows, const int64_t* ptr, const int32_t* idx, co
     S.nrows = nrows; S.nshort = nshort; S.nlong = nrows - nshort;
     S.nslices = (nshort + 31) / 32;
     S.slice_ptr.assign((size_t)S.nslices + 1, 0);
-    for (int64_t s = 0; s < S.nslices; ++s) {
-        int64_t w = 0;
-        for (int64_t r = 32 * s; r < std::min<int64_t>(32 * s + 32, nshort); ++r) {
-            int64_t o = perm[(size_t)r];
-            w = std::max(w, ptr[o + 1] - ptr[o]);
+    parallel_ranges(S.nslices, 1024, [&](int64_t sb, int64_t se) {
+        for (int64_t s = sb; s < se; ++s) {
+            int64_t w = 0;
+            for (int64_t r = 32 * s; r < std::min<int64_t>(32 * s + 32, nshort); ++r) {
+                int64_t o = perm[(size_t)r];
+                w = std::max(w, ptr[o + 1] - ptr[o]);
+            }
+            S.slice_ptr[(size_t)s + 1] = 32 * w;
         }
-        S.slice_ptr[(size_t)s + 1] = S.slice_ptr[(size_t)s] + 32 * w;
-    }
+    });
+    for (int64_t s = 0; s < S.nslices; ++s) S.slice_ptr[(size_t)s + 1] += S.slice_ptr[(size_t)s];
     const int64_t slots = S.slice_ptr[(size_t)S.nslices];
     S.col.assign((size_t)slots, 0); S.val.assign((size_t)slots, 0.0);
     if (want_src) S.src.assign((size_t)slots, -1);
-    for (int64_t r = 0; r < nshort; ++r) {
-        int64_t o = perm[(size_t)r], s = r >> 5, lane = r & 31, base = S.slice_ptr[(size_t)s];
-        for (int64_t p = ptr[o], t = 0; p < ptr[o + 1]; ++p, ++t) {
-            size_t k = (size_t)(base + t * 32 + lane);
-            S.col[k] = (int32_t)inv_other[(size_t)idx[p]];
-            S.val[k] = val[p];
-            if (want_src) S.src[k] = srcpos ? srcpos[p] : p;
+    parallel_ranges(nshort, 32768, [&](int64_t rb, int64_t re) {
+        for (int64_t r = rb; r < re; ++r) {
+            int64_t o = perm[(size_t)r], s = r >> 5, lane = r & 31, base = S.slice_ptr[(size_t)s];
+            for (int64_t p = ptr[o], t = 0; p < ptr[o + 1]; ++p, ++t) {
+                size_t k = (size_t)(base + t * 32 + lane);
+                S.col[k] = (int32_t)inv_other[(size_t)idx[p]];
+                S.val[k] = val[p];
+                if (want_src) S.src[k] = srcpos ? srcpos[p] : p;
+            }
         }
-    }
+    });
     S.lptr.assign((size_t)S.nlong + 1, 0);
     for (int64_t r = 0; r < S.nlong; ++r) {
         int64_t o = perm[(size_t)(nshort + r)];
@@ -183,19 +205,32 @@ inline std::string validate_csr(int64_t m, int64_t n, int64_t nnz, const int64_t
     if (row_ptr[0] != 0 || row_ptr[m] != nnz) return "row_ptr[0] != 0 or row_ptr[m] != nnz";
     if (nnz > 0 && (!col_idx || !val)) return "col_idx / val is NULL";
     if ((m > 0 && (!sense || !b)) || (n > 0 && (!c || !l || !u))) return "a vector argument is NULL";
-    std::vector<int64_t> stamp((size_t)std::max<int64_t>(n, 1), -1);
-    for (int64_t i = 0; i < m; ++i) {
-        if (row_ptr[i + 1] < row_ptr[i]) return "row_ptr is not monotone";
-        if (sense[i] != 'E' && sense[i] != 'G') return "sense must be 'E' or 'G'";
-        if (!std::isfinite(b[i])) return "b has a non-finite entry";
-        for (int64_t p = row_ptr[i]; p < row_ptr[i + 1]; ++p) {
-            int64_t j = col_idx[p];
-            if (j < 0 || j >= n) return "column index out of range";
-            if (stamp[(size_t)j] == i) return "duplicate entry within a row";
-            stamp[(size_t)j] = i;
-            if (!std::isfinite(val[p])) return "val has a non-finite entry";
+    for (int64_t i = 0; i < m; ++i)
+        if (row_ptr[i + 1] < row_ptr[i] || row_ptr[i + 1] > nnz) return "row_ptr is not monotone";
+    // rows are checked in parallel ranges, each with its own duplicate-detection stamps; the reported reason is
+    // that of the first range (in row order) that found one
+    const int kMaxRanges = 8;
+    std::vector<std::string> why_r((size_t)kMaxRanges);
+    const int64_t per = (m + kMaxRanges - 1) / kMaxRanges;
+    parallel_ranges(kMaxRanges, 1, [&](int64_t tb, int64_t te) {
+        std::vector<int64_t> stamp((size_t)std::max<int64_t>(n, 1), -1);
+        for (int64_t t = tb; t < te; ++t) {
+            const char* bad = nullptr;
+            for (int64_t i = t * per; i < std::min(m, (t + 1) * per) && !bad; ++i) {
+                if (sense[i] != 'E' && sense[i] != 'G') { bad = "sense must be 'E' or 'G'"; break; }
+                if (!std::isfinite(b[i])) { bad = "b has a non-finite entry"; break; }
+                for (int64_t p = row_ptr[i]; p < row_ptr[i + 1]; ++p) {
+                    int64_t j = col_idx[p];
+                    if (j < 0 || j >= n) { bad = "column index out of range"; break; }
+                    if (stamp[(size_t)j] == i) { bad = "duplicate entry within a row"; break; }
+                    stamp[(size_t)j] = i;
+                    if (!std::isfinite(val[p])) { bad = "val has a non-finite entry"; break; }
+                }
+            }
+            if (bad) why_r[(size_t)t] = bad;
         }
-    }
+    });
+    for (const std::string& w : why_r) if (!w.empty()) return w;
     for (int64_t j = 0; j < n; ++j) {
         if (!std::isfinite(c[j])) return "c has a non-finite entry";
         if (std::isnan(l[j]) || std::isnan(u[j])) return "a bound is NaN";
@@ -212,23 +247,32 @@ inline void build_problem(int64_t m, int64_t n, int64_t nnz, const int64_t* row_
     for (int64_t i = 0; i < m; ++i) lenr[(size_t)i] = row_ptr[i + 1] - row_ptr[i];
     for (int64_t p = 0; p < nnz; ++p) lenc[(size_t)col_idx[p]]++;
     int64_t ms = 0, ns = 0;
-    build_perm(lenr, window, long_thr, P.perm_r, P.inv_r, ms);
-    build_perm(lenc, window, long_thr, P.perm_c, P.inv_c, ns);
-    build_sell(m, row_ptr, col_idx, val, nullptr, P.perm_r, ms, P.inv_c, want_src, P.K);
+    {
+        std::thread t([&] { build_perm(lenr, window, long_thr, P.perm_r, P.inv_r, ms); });
+        build_perm(lenc, window, long_thr, P.perm_c, P.inv_c, ns);
+        t.join();
+    }
+    std::thread tk([&] { build_sell(m, row_ptr, col_idx, val, nullptr, P.perm_r, ms, P.inv_c, want_src, P.K); });
     // transpose
-    std::vector<int64_t> tptr((size_t)n + 1, 0), tsrc((size_t)nnz);
+    std::vector<int64_t> tptr((size_t)n + 1, 0), tsrc(want_src ? (size_t)nnz : 0);
     std::vector<int32_t> tidx((size_t)nnz);
     std::vector<double> tval((size_t)nnz);
     for (int64_t j = 0; j < n; ++j) tptr[(size_t)j + 1] = tptr[(size_t)j] + lenc[(size_t)j];
-    {
-        std::vector<int64_t> fill(tptr.begin(), tptr.end() - 1);
+    // counting sort by column, stable in the row index; each thread owns a range of columns, scans every entry and
+    // scatters only its own (its slice of the fill pointers stays in cache)
+    parallel_ranges(n, 65536, [&](int64_t jb, int64_t je) {
+        std::vector<int64_t> fill(tptr.begin() + jb, tptr.begin() + je);
         for (int64_t i = 0; i < m; ++i)
             for (int64_t p = row_ptr[i]; p < row_ptr[i + 1]; ++p) {
-                int64_t k = fill[(size_t)col_idx[p]]++;
-                tidx[(size_t)k] = (int32_t)i; tval[(size_t)k] = val[p]; tsrc[(size_t)k] = p;
+                const int64_t j = col_idx[p];
+                if (j < jb || j >= je) continue;
+                const int64_t k = fill[(size_t)(j - jb)]++;
+                tidx[(size_t)k] = (int32_t)i; tval[(size_t)k] = val[p];
+                if (want_src) tsrc[(size_t)k] = p;
             }
-    }
-    build_sell(n, tptr.data(), tidx.data(), tval.data(), tsrc.data(), P.perm_c, ns, P.inv_r, want_src, P.KT);
+    });
+    build_sell(n, tptr.data(), tidx.data(), tval.data(), want_src ? tsrc.data() : nullptr, P.perm_c, ns, P.inv_r, want_src, P.KT);
+    tk.join();
 }
 
 
