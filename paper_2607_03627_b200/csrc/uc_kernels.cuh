@@ -25,6 +25,10 @@ namespace ucpdhg {
 constexpr int kBlock = 256;          // threads per block of every row-parallel kernel
 constexpr int kWarps = kBlock / 32;  // = slices per block
 constexpr int kFinalBlock = 1024;    // threads of the single-block finalisers
+#ifndef UC_CHECK_MINB
+#define UC_CHECK_MINB 3
+#endif
+constexpr int kCheckMinBlocks = UC_CHECK_MINB;   // resident blocks per SM the check kernels are compiled for
 
 struct KktT { double rp2_s, rd2_s, rp2_u, rd2_u, pobj, dobj; };
 
@@ -84,7 +88,8 @@ struct Vecs {
     dd* partD;                   // [8][gridA]   check, dual side
     dd* partP;                   // [6][gridB]   check, primal side
     dd* partR;                   // [2][gridR]   restart distances
-    int gridA, gridB, gridR;     // one-block-per-256-rows grids of the check / restart kernels
+    int gridA, gridB, gridR;     // grids of the check kernels (persistent: grid-stride over the layout's blocks) and of
+                                 // the one-thread-per-element restart / flush kernels
     int gridPA, gridPB;          // persistent grids of the two attempt kernels
 };
 
@@ -182,19 +187,22 @@ __device__ __forceinline__ dd final_sum(const dd* part, int count, dd* red) {
 // they start first so that their sequential sums hide behind the sliced part), blocks
 // [nlblk, nlblk + nblk) own the sliced part (one thread per row).
 struct RowId { long long row; int slice; int lrow; bool owner; };
-__device__ __forceinline__ RowId my_row(const Sell& A) {
+// vb: the (virtual) block of the layout this thread block is working on -- blockIdx.x for the one-block-per-256-rows
+// kernels, a grid-stride counter for the check kernels
+__device__ __forceinline__ RowId my_row(const Sell& A, int vb) {
     RowId r; r.row = -1; r.slice = -1; r.lrow = -1; r.owner = false;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    if ((int)blockIdx.x >= A.nlblk) {
-        long long j = (long long)((int)blockIdx.x - A.nlblk) * kBlock + threadIdx.x;
+    if (vb >= A.nlblk) {
+        long long j = (long long)(vb - A.nlblk) * kBlock + threadIdx.x;
         int s = (int)(j >> 5);
         if (s < A.nslices) { r.slice = s; r.row = j; r.owner = j < A.nshort; }
     } else {
-        int lr = (int)blockIdx.x * kWarps + warp;
+        int lr = vb * kWarps + warp;
         if (lr < A.nlong) { r.lrow = lr; r.row = A.nshort + lr; r.owner = (lane == 0); }
     }
     return r;
 }
+__device__ __forceinline__ RowId my_row(const Sell& A) { return my_row(A, (int)blockIdx.x); }
 
 // --------------------------------------------------------------------------- SpMV row traversals
 // s[q] += sum_t val_t * g_t[q] over the entries of the row, left to right, multiply and add rounded
@@ -284,7 +292,7 @@ __global__ void __launch_bounds__(kBlock) k_flush(Vecs V, Ctrl* ctl) {
 // --------------------------------------------------------------------------- A11 check, dual side
 // per variable j (row of K~'), for z in {current, average}: rho = c - K~'y, lambda, r_d, c.x, bound
 // terms of the dual objective (R9).  partD rows: [rd2_s, rd2_u, pobj, dbound] x {cur, avg}.
-__global__ void __launch_bounds__(kBlock) k_check_dual(Sell KT, Vecs V, Ctrl* ctl) {
+__global__ void __launch_bounds__(kBlock, kCheckMinBlocks) k_check_dual(Sell KT, Vecs V, Ctrl* ctl) {
     __shared__ dd red[8 * 32];
     if (ld_flag(&ctl->done)) return;
     const int cur = ctl->cur;
@@ -292,11 +300,12 @@ __global__ void __launch_bounds__(kBlock) k_check_dual(Sell KT, Vecs V, Ctrl* ct
     const double* __restrict__ ycur = V.y[cur];
     const double* __restrict__ ysum = V.ysum;
     const int lane = threadIdx.x & 31;
-    const RowId r = my_row(KT);
     dd acc[8];
 #pragma unroll
     for (int q = 0; q < 8; ++q) acc[q] = dd{0.0, 0.0};
-    if (r.row >= 0) {
+    for (int vb = blockIdx.x; vb < KT.grid; vb += gridDim.x) {      // persistent blocks: ONE block reduction per block
+        const RowId r = my_row(KT, vb);
+        if (r.row < 0) continue;
         double g[2] = {0.0, 0.0};
         if (avg) row_dot<2>(KT, r, lane, g, [&](int c, double (&o)[2]) { o[0] = ycur[c]; o[1] = ysum[c] / w; });
         else { double g1[1] = {0.0}; row_dot<1>(KT, r, lane, g1, [&](int c, double (&o)[1]) { o[0] = ycur[c]; }); g[0] = g1[0]; }
@@ -313,10 +322,10 @@ __global__ void __launch_bounds__(kBlock) k_check_dual(Sell KT, Vecs V, Ctrl* ct
                 if (rj > 0.0 && lfin) lam = rj;
                 if (rj < 0.0 && ufin) lam = rj;
                 const double rd = rj - lam;
-                acc[4 * z + 0].hi = rd * rd;
-                acc[4 * z + 1].hi = (dc * rd) * (dc * rd);
-                acc[4 * z + 2].hi = cj * xj;
-                acc[4 * z + 3].hi = lam > 0.0 ? lj * lam : (lam < 0.0 ? uj * lam : 0.0);
+                acc[4 * z + 0] = dd_add_d(acc[4 * z + 0], rd * rd);
+                acc[4 * z + 1] = dd_add_d(acc[4 * z + 1], (dc * rd) * (dc * rd));
+                acc[4 * z + 2] = dd_add_d(acc[4 * z + 2], cj * xj);
+                acc[4 * z + 3] = dd_add_d(acc[4 * z + 3], lam > 0.0 ? lj * lam : (lam < 0.0 ? uj * lam : 0.0));
             }
         }
     }
@@ -327,7 +336,7 @@ __global__ void __launch_bounds__(kBlock) k_check_dual(Sell KT, Vecs V, Ctrl* ct
 
 // --------------------------------------------------------------------------- A11 check, primal side
 // per row i of K~: a = K~x - q, r_p, q.y (R9).  partP rows: [rp2_s, rp2_u, qy] x {cur, avg}.
-__global__ void __launch_bounds__(kBlock) k_check_primal(Sell K, Vecs V, Ctrl* ctl) {
+__global__ void __launch_bounds__(kBlock, kCheckMinBlocks) k_check_primal(Sell K, Vecs V, Ctrl* ctl) {
     __shared__ dd red[6 * 32];
     if (ld_flag(&ctl->done)) return;
     const int cur = ctl->cur;
@@ -335,11 +344,12 @@ __global__ void __launch_bounds__(kBlock) k_check_primal(Sell K, Vecs V, Ctrl* c
     const double* __restrict__ xcur = V.x[cur];
     const double* __restrict__ xsum = V.xsum;
     const int lane = threadIdx.x & 31;
-    const RowId r = my_row(K);
     dd acc[6];
 #pragma unroll
     for (int q = 0; q < 6; ++q) acc[q] = dd{0.0, 0.0};
-    if (r.row >= 0) {
+    for (int vb = blockIdx.x; vb < K.grid; vb += gridDim.x) {       // persistent blocks: ONE block reduction per block
+        const RowId r = my_row(K, vb);
+        if (r.row < 0) continue;
         double a[2] = {0.0, 0.0};
         if (avg) row_dot<2>(K, r, lane, a, [&](int c, double (&o)[2]) { o[0] = xcur[c]; o[1] = xsum[c] / w; });
         else { double a1[1] = {0.0}; row_dot<1>(K, r, lane, a1, [&](int c, double (&o)[1]) { o[0] = xcur[c]; }); a[0] = a1[0]; }
@@ -352,9 +362,9 @@ __global__ void __launch_bounds__(kBlock) k_check_primal(Sell K, Vecs V, Ctrl* c
                 const double ai = a[z] - qi;
                 const double yi = z ? V.ysum[i] / w : V.y[cur][i];
                 const double rp = isg ? (ai < 0.0 ? ai : 0.0) : ai;
-                acc[3 * z + 0].hi = rp * rp;
-                acc[3 * z + 1].hi = (dr * rp) * (dr * rp);
-                acc[3 * z + 2].hi = qi * yi;
+                acc[3 * z + 0] = dd_add_d(acc[3 * z + 0], rp * rp);
+                acc[3 * z + 1] = dd_add_d(acc[3 * z + 1], (dr * rp) * (dr * rp));
+                acc[3 * z + 2] = dd_add_d(acc[3 * z + 2], qi * yi);
             }
         }
     }

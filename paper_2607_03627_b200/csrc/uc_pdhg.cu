@@ -189,8 +189,8 @@ void launch_primal(uc_lp* lp, cudaStream_t st) { launch_pdl(k_primal, lp->V.grid
 void launch_dual(uc_lp* lp, cudaStream_t st) { launch_pdl(k_dual, lp->V.gridPB, sizeof(DualSmem), st, lp->K, lp->V, lp->ctl); }
 void launch_attempt(uc_lp* lp, cudaStream_t st) { launch_primal(lp, st); launch_dual(lp, st); }
 void launch_kkt(uc_lp* lp, cudaStream_t st, int mode) {
-    k_check_dual<<<lp->KT.grid, kBlock, 0, st>>>(lp->KT, lp->V, lp->ctl);
-    k_check_primal<<<lp->K.grid, kBlock, 0, st>>>(lp->K, lp->V, lp->ctl);
+    k_check_dual<<<lp->V.gridA, kBlock, 0, st>>>(lp->KT, lp->V, lp->ctl);
+    k_check_primal<<<lp->V.gridB, kBlock, 0, st>>>(lp->K, lp->V, lp->ctl);
     k_check_finalize<<<1, kFinalBlock, 0, st>>>(lp->V, lp->ctl, mode);
 }
 void launch_check(uc_lp* lp, cudaStream_t st) {
@@ -348,7 +348,13 @@ int uc_lp_create(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, cons
         lp->qs = lp->dalloc<double>((size_t)m); lp->isG = lp->dalloc<unsigned char>((size_t)m);
         lp->Dr = lp->dalloc<double>((size_t)m); lp->Dc = lp->dalloc<double>((size_t)n);
         V.c = lp->cs; V.l = lp->ls; V.u = lp->us; V.q = lp->qs; V.isG = lp->isG; V.Dr = lp->Dr; V.Dc = lp->Dc;
-        V.gridA = lp->KT.grid; V.gridB = lp->K.grid; V.gridR = std::max(1, cdiv(n + m, kBlock));
+        V.gridR = std::max(1, cdiv(n + m, kBlock));
+        {   // check kernels: persistent blocks, kCheckMinBlocks per SM, grid-stride over the layout's 256-row blocks
+            int sms = 0;
+            CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+            const int cap = kCheckMinBlocks * std::max(sms, 1);
+            V.gridA = std::max(1, std::min(cap, lp->KT.grid)); V.gridB = std::max(1, std::min(cap, lp->K.grid));
+        }
         V.gridPA = gridPA; V.gridPB = gridPB;
         CK(cudaFuncSetAttribute(k_primal, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(PrimalSmem)));
         CK(cudaFuncSetAttribute(k_dual, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(DualSmem)));
