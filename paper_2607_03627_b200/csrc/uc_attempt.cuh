@@ -146,7 +146,7 @@ __device__ __forceinline__ void dispatch_nt(int nt, F f) {
 template <class Ring, class GT, class FD, class FV, class FC>
 __device__ __forceinline__ bool warp_pipeline(const Sell& A, Ring& R, int gw, int lane, const GT* const& gsrc,
                                               uint64_t pol_first, FD dep_ready, FV issue_vecs, FC compute) {
-    const int J = A.steps_per_warp;
+    int J = A.steps_per_warp;                                      // shrinks to this warp's own count at its end marker
     const long long GW = A.sched_warps;
     auto load_desc = [&](int k) -> int4 {
         return k < J ? __ldg(reinterpret_cast<const int4*>(A.steps + (long long)k * GW + gw)) : make_int4(0, 0, 0, 0);
@@ -169,6 +169,7 @@ __device__ __forceinline__ bool warp_pipeline(const Sell& A, Ring& R, int gw, in
         const int dx_ = __shfl_sync(0xffffffffu, dcur.x, src_lane), dy_ = __shfl_sync(0xffffffffu, dcur.y, src_lane);
         const int row_a = __shfl_sync(0xffffffffu, dcur.z, src_lane), info_a = __shfl_sync(0xffffffffu, dcur.w, src_lane);
         const long long eb_a = ((long long)(unsigned)dx_) | ((long long)dy_ << 32);
+        if (info_a & 64) J = min(J, ka);
         if (lane < (info_a & 7) * 8) cp_stream16(&R.col[sa][lane * 4], A.col + eb_a + lane * 4, pol_first);
         // ---- B: values, vectors and gathers of step kb = j + kDB (its indices landed kDB commits ago)
         const long long eb = qa_e[0]; const int info_b = qa_i[0], row_b = qa_r[0];

@@ -30,7 +30,8 @@ struct StepDesc {
     long long ebase;   // first stored entry of the chunk in the sliced-ELL arrays
     int row0;          // first row of the slice
     int info;          // bits 0-2: entries per row in this chunk (0 = padding step: nothing to do); bit 4: first chunk
-                       // of its slice; bit 5: last chunk of its slice (the update is applied)
+                       // of its slice; bit 5: last chunk of its slice (the update is applied); bit 6: the warp has no
+                       // further steps (set on its first padding step)
 };
 static_assert(sizeof(StepDesc) == 16, "StepDesc layout");
 
@@ -65,9 +66,10 @@ struct HostSell {
 };
 
 // Static schedule of the persistent attempt kernels for `warps` consumer warps in total.  Slices are taken in
-// ascending order and each goes to the warp with the fewest steps so far (ties: lowest warp), so that the
-// warps' step counts differ by at most one slice's worth while, at any moment, all warps work on neighbouring
-// slices (DRAM pages and L2 lines are shared).  A warp takes its slices in ascending order, each as
+// ascending order and each goes to the warp with the least estimated work so far (ties: lowest warp), so that
+// the warps finish together while, at any moment, all warps work on neighbouring slices (DRAM pages and L2
+// lines are shared).  The estimate is in units of ~100 cycles from the measured per-step breakdown
+// (DESIGN.md section 7): 7 per step + 1.3 per entry per row + 4 for the step that applies the update.  A warp takes its slices in ascending order, each as
 // ceil(width / kChunkT) steps.  Stored step-major, steps[j * warps + w], padded with empty steps to the
 // longest warp, so that step j of all warps is one coalesced read.  The assignment is fixed at create time:
 // solves are reproducible bit for bit.
@@ -84,8 +86,9 @@ inline void build_schedule(HostSell& S, int64_t warps) {
             const int64_t wd = (S.slice_ptr[(size_t)s + 1] - S.slice_ptr[(size_t)s]) / 32;
             Load l = heap.top(); heap.pop();
             owner[(size_t)s] = (int32_t)l.second;
-            l.first += std::max<int64_t>(1, (wd + kChunkT - 1) / kChunkT);
-            count[(size_t)l.second] = l.first;
+            const int64_t nch = std::max<int64_t>(1, (wd + kChunkT - 1) / kChunkT);
+            l.first += 70 * nch + 13 * wd + 40;
+            count[(size_t)l.second] += nch;
             heap.push(l);
         }
     }
@@ -107,6 +110,8 @@ inline void build_schedule(HostSell& S, int64_t warps) {
             S.steps[(size_t)(count[(size_t)w]++ * warps + w)] = d;
         }
     }
+    for (int64_t w = 0; w < warps; ++w)
+        if (count[(size_t)w] < J) S.steps[(size_t)(count[(size_t)w] * warps + w)].info = 64;
 }
 
 // new -> old permutation: short rows in length-sorted windows, long rows last.
