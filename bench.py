@@ -42,8 +42,8 @@ def algorithmic_bytes(m, n, nnz):
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the attempt kernels on config 3, from the one
-# `ncu --set full` capture summarised in profiles/r01c_summary.md (cold L2 per replay; bytes)
-NCU_TRAFFIC_CONFIG3 = {"k_primal": 185.75e6 + 12.06e6, "k_dual": 161.96e6 + 5.21e6, "source": "profiles/r01c_summary.md"}
+# `ncu --set full` capture summarised in profiles/r01d_summary.md (cold L2 per replay; bytes)
+NCU_TRAFFIC_CONFIG3 = {"k_primal": 185.74e6 + 11.84e6, "k_dual": 162.19e6 + 4.21e6, "source": "profiles/r01d_summary.md"}
 
 
 def load_peaks():
