@@ -13,7 +13,7 @@
 //     16 KB tiles, hopeless for the 2 KB vector segments and ~1 KB index/value chunks this path is made of;
 //   * a coalesced cp.async (LDGSTS.128) costs ~8 cycles and holds no register while in flight;
 //   * divergent gathers run at ~1000 gathers/us/SM from 4 issuing warps but ~1500 from 8 or more.
-// Hence: persistent CTAs (two per SM) of kAttWarps CONSUMER warps, every one of which runs its own
+// Hence: persistent CTAs (one per SM) of kAttWarps CONSUMER warps, every one of which runs its own
 // three-stage software pipeline on its own shared-memory rings, with NO block-level synchronisation inside
 // the loop.  The unit of work is a STEP (uc_format.hpp): up to kChunkT entries per row of one slice (32 rows,
 // one per lane).  For its step j a warp has, in flight at the same time,
@@ -44,10 +44,10 @@ namespace ucpdhg {
 
 // build-time tunables (-DUC_...): the defaults are the measured optimum on config 3 (profiles/)
 #ifndef UC_ATT_WARPS
-#define UC_ATT_WARPS 7
+#define UC_ATT_WARPS 15
 #endif
 #ifndef UC_CTAS_PER_SM
-#define UC_CTAS_PER_SM 2
+#define UC_CTAS_PER_SM 1
 #endif
 #ifndef UC_DB
 #define UC_DB 1
@@ -148,10 +148,10 @@ __device__ __forceinline__ bool warp_pipeline(const Sell& A, Ring& R, int gw, in
                                               uint64_t pol_first, FD dep_ready, FV issue_vecs, FC compute) {
     int J = A.steps_per_warp;                                      // shrinks to this warp's own count at its end marker
     const long long GW = A.sched_warps;
-    auto load_desc = [&](int k) -> int4 {
-        return k < J ? __ldg(reinterpret_cast<const int4*>(A.steps + (long long)k * GW + gw)) : make_int4(0, 0, 0, 0);
+    auto load_desc = [&](int k) -> int2 {
+        return k < J ? __ldg(reinterpret_cast<const int2*>(A.steps + (long long)k * GW + gw)) : make_int2(0, 0);
     };
-    int4 dcur = load_desc(lane), dnxt = load_desc(32 + lane);
+    int2 dcur = load_desc(lane), dnxt = load_desc(32 + lane);
     long long qa_e[kDA - kDB]; int qa_i[kDA - kDB], qa_r[kDA - kDB];     // A -> B
     int qb_i[kDB], qb_r[kDB];                                            // B -> C
 #pragma unroll
@@ -166,10 +166,10 @@ __device__ __forceinline__ bool warp_pipeline(const Sell& A, Ring& R, int gw, in
         const int ka = j + kDA;
         if (ka >= 32 && (ka & 31) == 0) { dcur = dnxt; dnxt = load_desc(ka + 32 + lane); }
         const int src_lane = ka & 31;
-        const int dx_ = __shfl_sync(0xffffffffu, dcur.x, src_lane), dy_ = __shfl_sync(0xffffffffu, dcur.y, src_lane);
-        const int row_a = __shfl_sync(0xffffffffu, dcur.z, src_lane), info_a = __shfl_sync(0xffffffffu, dcur.w, src_lane);
-        const long long eb_a = ((long long)(unsigned)dx_) | ((long long)dy_ << 32);
-        if (info_a & 64) J = min(J, ka);
+        const unsigned w0 = (unsigned)__shfl_sync(0xffffffffu, dcur.x, src_lane);
+        const int row_a = __shfl_sync(0xffffffffu, dcur.y, src_lane), info_a = (int)(w0 >> 26);
+        const long long eb_a = (long long)(w0 & 0x3ffffffu) << 5;
+        if (info_a & kStepEnd) J = min(J, ka);
         if (lane < (info_a & 7) * 8) cp_stream16(&R.col[sa][lane * 4], A.col + eb_a + lane * 4, pol_first);
         // ---- B: values, vectors and gathers of step kb = j + kDB (its indices landed kDB commits ago)
         const long long eb = qa_e[0]; const int info_b = qa_i[0], row_b = qa_r[0];
@@ -184,7 +184,7 @@ __device__ __forceinline__ bool warp_pipeline(const Sell& A, Ring& R, int gw, in
                 const int p = k * 32 + lane;                       // 16-byte piece of the value chunk
                 if (p < nt * 16) cp_stream16(&D.val[p * 2], A.val + eb + p * 2, pol_first);
             }
-            if (info_b & 32) issue_vecs(D, row_b);
+            if (info_b & kStepLast) issue_vecs(D, row_b);
             dispatch_nt(nt, [&](auto n) {
                 int c[decltype(n)::value];
 #pragma unroll
@@ -294,9 +294,9 @@ __global__ void __launch_bounds__(kAttemptThreads, kCtasPerSm) k_primal(Sell KT,
                     if (vok[k]) cp_stream16(&D.vec[0][0] + voff[k], vsrc[k] + row0, pol.first);
             },
             [&](auto& D, int info, int row0) {
-                if (info & 16) g[0] = 0.0;
+                if (info & kStepFirst) g[0] = 0.0;
                 step_sum<1>(D.val, D.gv, info & 7, lane, g);
-                if (info & 32) {
+                if (info & kStepLast) {
                     const long long j = (long long)row0 + lane;
                     if (j < KT.nshort) {
                         const PrimalRow pr{D.vec[0][lane], D.vec[1][lane], D.vec[2][lane], D.vec[3][lane], pend ? D.vec[4][lane] : 0.0};
@@ -372,9 +372,9 @@ __global__ void __launch_bounds__(kAttemptThreads, kCtasPerSm) k_dual(Sell K, Ve
                 if (lane == 16 || lane == 17) cp_stream16(&D.bvec[(lane - 16) * 16], V.isG + row0 + (lane - 16) * 16, pol.first);
             },
             [&](auto& D, int info, int row0) {
-                if (info & 16) { kx[0] = 0.0; kx[1] = 0.0; }
+                if (info & kStepFirst) { kx[0] = 0.0; kx[1] = 0.0; }
                 step_sum<2>(D.val, D.gv, info & 7, lane, kx);
-                if (info & 32) {
+                if (info & kStepLast) {
                     const long long i = (long long)row0 + lane;
                     if (i < K.nshort) {
                         const DualRow dr{D.vec[0][lane], D.vec[1][lane], pend ? D.vec[2][lane] : 0.0, (int)D.bvec[lane]};

@@ -24,16 +24,17 @@ namespace ucpdhg {
 
 // One step of the warp-private pipelines of the persistent attempt kernels (uc_attempt.cuh): a chunk of at
 // most kChunkT entries per row of one slice.  A slice wider than kChunkT is a run of consecutive steps of
-// the same warp, the row sums carried in registers from one to the next.  16 bytes.
+// the same warp, the row sums carried in registers from one to the next.  8 bytes.
 constexpr int kChunkT = 4;
 struct StepDesc {
-    long long ebase;   // first stored entry of the chunk in the sliced-ELL arrays
-    int row0;          // first row of the slice
-    int info;          // bits 0-2: entries per row in this chunk (0 = padding step: nothing to do); bit 4: first chunk
-                       // of its slice; bit 5: last chunk of its slice (the update is applied); bit 6: the warp has no
-                       // further steps (set on its first padding step)
+    uint32_t w0;       // bits 0-25: (first stored entry of the chunk in the sliced-ELL arrays) / 32; bits 26-31: info
+    int32_t row0;      // first row of the slice
 };
-static_assert(sizeof(StepDesc) == 16, "StepDesc layout");
+// info: bits 0-2 entries per row in this chunk (0 = padding step: nothing to do)
+constexpr int kStepFirst = 8;    // first chunk of its slice
+constexpr int kStepLast = 16;    // last chunk of its slice (the update is applied)
+constexpr int kStepEnd = 32;     // the warp has no further steps (set on its first padding step)
+static_assert(sizeof(StepDesc) == 8, "StepDesc layout");
 
 // f(begin, end) over [0, n) on up to 8 host threads (uc_lp_create is a one-time cost, but it is inside the
 // end-to-end time: the layouts of a 6M-entry matrix take ~0.5 s on one core)
@@ -95,7 +96,7 @@ inline void build_schedule(HostSell& S, int64_t warps) {
     int64_t J = 0;
     for (int64_t c : count) J = std::max(J, c);
     S.steps_per_warp = J;
-    S.steps.assign((size_t)(J * warps), StepDesc{0, 0, 0});
+    S.steps.assign((size_t)(J * warps), StepDesc{0u, 0});
     std::fill(count.begin(), count.end(), 0);
     for (int64_t s = 0; s < S.nslices; ++s) {
         const int64_t wd = (S.slice_ptr[(size_t)s + 1] - S.slice_ptr[(size_t)s]) / 32;
@@ -103,15 +104,15 @@ inline void build_schedule(HostSell& S, int64_t warps) {
         const int64_t w = owner[(size_t)s];
         for (int64_t c = 0; c < nch; ++c) {
             StepDesc d;
-            d.ebase = S.slice_ptr[(size_t)s] + 32 * kChunkT * c;
-            d.row0 = (int)(32 * s);
             const int64_t nt = std::min<int64_t>(kChunkT, wd - kChunkT * c);
-            d.info = (int)std::max<int64_t>(nt, 0) | (c == 0 ? 16 : 0) | (c == nch - 1 ? 32 : 0);
+            const uint32_t info = (uint32_t)std::max<int64_t>(nt, 0) | (c == 0 ? kStepFirst : 0) | (c == nch - 1 ? kStepLast : 0);
+            d.w0 = (uint32_t)((S.slice_ptr[(size_t)s] + 32 * kChunkT * c) >> 5) | (info << 26);   // slots < 2^31 (checked at create)
+            d.row0 = (int32_t)(32 * s);
             S.steps[(size_t)(count[(size_t)w]++ * warps + w)] = d;
         }
     }
     for (int64_t w = 0; w < warps; ++w)
-        if (count[(size_t)w] < J) S.steps[(size_t)(count[(size_t)w] * warps + w)].info = 64;
+        if (count[(size_t)w] < J) S.steps[(size_t)(count[(size_t)w] * warps + w)].w0 = (uint32_t)kStepEnd << 26;
 }
 
 // new -> old permutation: short rows in length-sorted windows, long rows last.

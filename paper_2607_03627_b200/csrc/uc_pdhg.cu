@@ -252,9 +252,9 @@ void destroy_impl(uc_lp* lp) {
 
 int64_t bytes_per_attempt(const uc_lp* lp) {
     // what one attempt streams in THIS layout: matrix slots (12 B each, padding included),
-    // step descriptors (16 B per scheduled step, padding steps included), and per variable 8 (x) + 24 (c,l,u) + 16 (xsum r/w) + 8 (x') + 16 ({xbar,dx}) + 16
+    // step descriptors (8 B per scheduled step, padding steps included), and per variable 8 (x) + 24 (c,l,u) + 16 (xsum r/w) + 8 (x') + 16 ({xbar,dx}) + 16
     // (gather of the pair) = 88 B, per row 8 (y) + 8 (q) + 1 (sense) + 16 (ysum r/w) + 8 (y') + 8 (gather) = 49 B
-    return 12 * (lp->k_slots + lp->kt_slots + lp->k_long_nnz + lp->kt_long_nnz) + 16 * ((int64_t)lp->K.steps_per_warp * lp->K.sched_warps + (int64_t)lp->KT.steps_per_warp * lp->KT.sched_warps) +
+    return 12 * (lp->k_slots + lp->kt_slots + lp->k_long_nnz + lp->kt_long_nnz) + 8 * ((int64_t)lp->K.steps_per_warp * lp->K.sched_warps + (int64_t)lp->KT.steps_per_warp * lp->KT.sched_warps) +
            88 * lp->n + 49 * lp->m;
 }
 
@@ -318,6 +318,8 @@ int uc_lp_create(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, cons
         // A0 / A1: layouts (host), upload
         HostProblem P;
         build_problem(m, n, nnz, row_ptr, col_idx, val, opt.sell_window, opt.long_row_threshold, opt.keep_source_map != 0, P);
+        if (P.K.col.size() >= (size_t)1 << 31 || P.KT.col.size() >= (size_t)1 << 31)
+            throw std::bad_alloc();                      // the step descriptors address stored entries / 32 in 26 bits
         int gridPA = 1, gridPB = 1;
         {   // persistent grids of the attempt kernels: kCtasPerSm CTAs per SM, never more CTAs than work; the static
             // schedule gives slice s to consumer warp s % (grid * kAttWarps)
