@@ -104,7 +104,7 @@ typedef struct {
 } uc_check_record;
 
 typedef struct {
-    int64_t iter_limit;       /* 100000 */
+    int64_t iter_limit;       /* 100000  PAPER.md l.66.  Any size: per-attempt tables grow while the solve runs */
     double eps_rel;           /* 1e-4    PAPER.md l.91 "convergence tolerance" */
     double eps_abs;           /* 1e-4 (= eps_rel, R12); 1e-5 reproduces the paper's extra knob (l.66) */
     double time_limit_s;      /* +inf */

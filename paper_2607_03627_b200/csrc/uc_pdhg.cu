@@ -160,15 +160,40 @@ void precondition(uc_lp* lp, cudaStream_t st) {
 // The factors of the step rule depend on the attempt counter only.  They are tabulated on the host with
 // the C library's pow (correctly rounded in all but freak cases), because one ulp in eta is amplified
 // exponentially by the adaptive rule and CUDA's pow is only 2-ulp accurate.
-void ensure_powtab(uc_lp* lp, long long limit) {
-    if (limit <= lp->powtab_len) return;
-    long long len = std::max<long long>(limit, 4096);
-    std::vector<double2> h((size_t)len);
-    for (long long k = 1; k <= len; ++k) h[(size_t)k - 1] = make_double2(std::pow((double)(k + 1), -0.6), std::pow((double)(k + 1), -0.3));
+// The table covers the attempts the device can reach before the host looks again, not iter_limit: it starts at
+// kPowtabStart entries and the launch loop doubles it ahead of the attempt counter (grow_powtab), so a huge
+// iteration limit costs nothing up front and a cancel is never stuck behind table building.
+constexpr long long kPowtabStart = 1 << 18;
+void fill_powtab(std::vector<double2>& h, long long from, long long to) {     // entries for attempts from+1 .. to
+    h.resize((size_t)(to - from));
+    for (long long k = from + 1; k <= to; ++k) h[(size_t)(k - from - 1)] = make_double2(std::pow((double)(k + 1), -0.6), std::pow((double)(k + 1), -0.3));
+}
+void ensure_powtab(uc_lp* lp, long long need) {
+    need = std::max<long long>(need, 4096);
+    if (need <= lp->powtab_len) return;
+    std::vector<double2> h;
+    fill_powtab(h, 0, need);
     if (lp->powtab) { cudaFree(lp->powtab); lp->powtab = nullptr; lp->powtab_len = 0; }
-    CK(cudaMalloc((void**)&lp->powtab, sizeof(double2) * (size_t)len));
-    CK(cudaMemcpy(lp->powtab, h.data(), sizeof(double2) * (size_t)len, cudaMemcpyHostToDevice));
-    lp->powtab_len = len;
+    CK(cudaMalloc((void**)&lp->powtab, sizeof(double2) * (size_t)need));
+    CK(cudaMemcpy(lp->powtab, h.data(), sizeof(double2) * (size_t)need, cudaMemcpyHostToDevice));
+    lp->powtab_len = need;
+}
+// Grow the table to at least `need` entries while a solve is in flight on `st`: the new table is complete before
+// the pointer in Ctrl is switched (stream-ordered, i.e. between two graph launches); the old table is kept in
+// `retired` until the solve has drained the stream.
+void grow_powtab(uc_lp* lp, long long need, long long limit, cudaStream_t st, std::vector<double2*>& retired) {
+    if (need <= lp->powtab_len) return;
+    const long long len = std::min<long long>(limit, std::max<long long>(need, 2 * lp->powtab_len));
+    std::vector<double2> h;
+    fill_powtab(h, lp->powtab_len, len);
+    double2* nt = nullptr;
+    CK(cudaMalloc((void**)&nt, sizeof(double2) * (size_t)len));
+    CK(cudaMemcpyAsync(nt, lp->powtab, sizeof(double2) * (size_t)lp->powtab_len, cudaMemcpyDeviceToDevice, st));
+    CK(cudaMemcpyAsync(nt + lp->powtab_len, h.data(), sizeof(double2) * h.size(), cudaMemcpyHostToDevice, st));
+    CK(cudaStreamSynchronize(st));                    // `h` is pageable and goes out of scope; the loop keeps 2 launches queued
+    retired.push_back(lp->powtab);
+    lp->powtab = nt; lp->powtab_len = len;
+    CK(cudaMemcpyAsync(&lp->ctl->powtab, &lp->powtab, sizeof(double2*), cudaMemcpyHostToDevice, st));
 }
 
 // The two attempt kernels are launched with programmatic stream serialization (PDL): a kernel's prologue
@@ -204,7 +229,7 @@ constexpr int kCheckLaunches = 6;
 // R2: control block, initial point, KKT components of the restart point z^0 (4 launches); synchronises `st`.
 void start_run(uc_lp* lp, const uc_pdhg_params& prm, cudaStream_t st, long long limit, bool fixed,
                const double* dx0, const double* dy0, uc_attempt_record* d_att, uc_check_record* d_chk) {
-    ensure_powtab(lp, limit);
+    ensure_powtab(lp, std::min<long long>(limit, kPowtabStart));
     Ctrl h{};
     h.eta = lp->eta0; h.omega = lp->omega0; h.eta_prev = 0.0; h.w = 0.0; h.mu_prev = INFINITY;
     h.limit = limit; h.fixed = fixed ? 1 : 0; h.status = UC_ITERATION_LIMIT;
@@ -509,7 +534,9 @@ static int solve_impl(uc_lp* lp, const uc_pdhg_params* pin, double* x_out, doubl
         const int depth = 2;
         bool done = false;
         long long b = 0;
+        std::vector<double2*> retired_powtabs;
         for (; b < nblocks && !done; ++b) {
+            if ((b + 8) * ce > lp->powtab_len && lp->powtab_len < limit) grow_powtab(lp, std::min<long long>(limit, (b + 8) * ce), limit, st, retired_powtabs);
             CK(cudaGraphLaunch(lp->exec, st));
             launches += lp->graph_nodes;
             CK(cudaEventRecord(lp->ev[b % depth], st));
@@ -522,6 +549,7 @@ static int solve_impl(uc_lp* lp, const uc_pdhg_params* pin, double* x_out, doubl
         CK(cudaStreamSynchronize(st));
         done = ((volatile HostStatus*)lp->h_status)->done != 0;
         if (!done && rem > 0) {
+            grow_powtab(lp, limit, limit, st, retired_powtabs);
             for (long long r = 0; r < rem; ++r) launch_attempt(lp, st);
             launches += 2 * rem;
             if (!fixed) { launch_check(lp, st); launches += kCheckLaunches; }
@@ -529,6 +557,7 @@ static int solve_impl(uc_lp* lp, const uc_pdhg_params* pin, double* x_out, doubl
             done = ((volatile HostStatus*)lp->h_status)->done != 0;
         }
         CK(cudaEventRecord(lp->ev_t1, st));
+        for (double2* t : retired_powtabs) cudaFree(t);     // the stream has drained: nobody reads the old tables
         if (!done) {                                       // fixed-iteration end (R14) or iter_limit = 0: report only
             launch_kkt(lp, st, kModeReport);
             launches += 3;

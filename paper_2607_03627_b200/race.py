@@ -1,0 +1,111 @@
+"""Algorithm 1 of the paper: race the GPU PDHG solver against a CPU LP solver on the same
+relaxed problem and terminate the loser.
+
+    1  partition the CPU cores between the two pipelines                     (l.70; here: `cpu_threads`)
+    2  start pipeline 1: PDHG on the GPU                                      (l.74)
+    3  start pipeline 2: the CPU competitor                                   (l.77)
+    4  while neither has converged: sleep `poll_s` (0.5 s in the paper, l.81)
+    5  terminate the other solver, return the winner's solution               (l.82-85)
+
+The paper's competitor is Gurobi's barrier; it is not available here, so the competitor is any callable that
+solves the LP on the host (the tests use HiGHS through scipy).  It runs in a child PROCESS, because "terminate"
+has to work on a solver that offers no cancel hook; the GPU side is stopped with uc_pdhg_cancel, which is what
+that entry point exists for.  Crossover, simplex clean-up and branch-and-bound (the rest of both pipelines) are
+out of scope.
+"""
+from __future__ import annotations
+
+import multiprocessing as mp
+import threading
+import time
+from dataclasses import dataclass, field
+from typing import Any, Callable, Optional
+
+from . import binding as _b
+
+
+@dataclass
+class RaceResult:
+    winner: str                      # "gpu_pdhg" or "cpu"
+    objective: float
+    seconds: float                   # wall time until the winner was seen (poll granularity included)
+    gpu: Optional[Any] = None        # Solution of the GPU side (status CANCELLED if it lost)
+    cpu: Optional[Any] = None        # whatever the competitor returned (None if it was terminated)
+    gpu_seconds: Optional[float] = None      # when the GPU side returned, from the start of the race
+    cpu_seconds: Optional[float] = None      # when the competitor returned (None if terminated)
+    cancel_latency_s: Optional[float] = None  # uc_pdhg_cancel -> uc_pdhg_solve returned (only if the GPU lost)
+    polls: int = 0
+    log: list = field(default_factory=list)
+
+
+def _child(fn, args, q):
+    try:
+        q.put(("ok", fn(*args)))
+    except BaseException as e:      # the parent must never wait for a dead child
+        q.put(("error", repr(e)))
+
+
+def race(handle: "_b.UcLp", competitor: Callable[..., Any], competitor_args: tuple = (), *,
+         competitor_objective: Callable[[Any], float] = lambda r: float(r),
+         poll_s: float = 0.5, solve_kwargs: Optional[dict] = None, mp_context: str = "fork") -> RaceResult:
+    """Run Algorithm 1.  `handle` is a created UcLp (the LP is already on the GPU: presolve and model building
+    are upstream of this library); `competitor(*competitor_args)` solves the same LP on the host and returns
+    something `competitor_objective` can turn into the optimal objective value."""
+    solve_kwargs = dict(solve_kwargs or {})
+    t0 = time.perf_counter()
+    box: dict = {}
+
+    def gpu_side():
+        box["sol"] = handle.solve(**solve_kwargs)
+        box["t"] = time.perf_counter() - t0
+
+    ctx = mp.get_context(mp_context)
+    q = ctx.Queue()
+    proc = ctx.Process(target=_child, args=(competitor, competitor_args, q), daemon=True)
+    th = threading.Thread(target=gpu_side, daemon=True)
+    th.start()                       # line 2: pipeline 1
+    proc.start()                     # line 3: pipeline 2
+    res = RaceResult(winner="", objective=float("nan"), seconds=0.0)
+    cpu_msg = None
+    while True:                      # line 4
+        gpu_done = not th.is_alive()
+        if cpu_msg is None and not q.empty():
+            cpu_msg = q.get()
+            res.cpu_seconds = time.perf_counter() - t0
+        if gpu_done or (cpu_msg is not None and cpu_msg[0] == "ok"):
+            break
+        if cpu_msg is not None and cpu_msg[0] == "error" and "competitor failed" not in " ".join(res.log):
+            res.log.append("competitor failed: " + cpu_msg[1])     # keep waiting for the GPU side
+        time.sleep(poll_s)
+        res.polls += 1
+    res.seconds = time.perf_counter() - t0
+    gpu_ok = (not th.is_alive()) and box.get("sol") is not None and box["sol"].status == _b.OPTIMAL
+    cpu_ok = cpu_msg is not None and cpu_msg[0] == "ok"
+    if gpu_ok and (not cpu_ok or box["t"] <= (res.cpu_seconds or float("inf"))):
+        # line 5, GPU first: terminate the competitor
+        res.winner = "gpu_pdhg"
+        res.objective = box["sol"].primal_obj
+        if proc.is_alive():
+            proc.terminate()
+        res.log.append("competitor terminated")
+    elif cpu_ok:
+        # line 5, CPU first: stop the GPU solver through its cancel hook and time how long it takes to return
+        res.winner = "cpu"
+        res.cpu = cpu_msg[1]
+        res.objective = competitor_objective(cpu_msg[1])
+        if th.is_alive():
+            tc = time.perf_counter()
+            handle.cancel()
+            th.join()
+            res.cancel_latency_s = time.perf_counter() - tc
+            res.log.append("uc_pdhg_cancel sent")
+    else:
+        th.join()
+        proc.join(timeout=1.0)
+        raise RuntimeError(f"neither solver converged: gpu {box.get('sol')}, cpu {cpu_msg}")
+    proc.join(timeout=5.0)
+    if th.is_alive():
+        th.join()
+    res.gpu = box.get("sol")
+    res.gpu_seconds = box.get("t")
+    return res

@@ -291,3 +291,17 @@ def test_solves_are_reproducible_bit_for_bit():
         c = h2.solve(fixed_iterations=300)
     np.testing.assert_array_equal(a.x, b.x); np.testing.assert_array_equal(a.y, b.y)
     np.testing.assert_array_equal(a.x, c.x); np.testing.assert_array_equal(a.y, c.y)
+
+
+def test_long_run_crosses_step_rule_table_growth():
+    """The {(k+1)^-0.6, (k+1)^-0.3} table of R5 starts at 2^18 entries and is doubled by the launch loop while the
+    solve is in flight: 300,000 attempts cross that switch; the step sizes must stay those of the oracle."""
+    lp = uc_config(0)
+    F = 300_000
+    so = oracle.solve(lp, fixed_iterations=F, trace_attempts=F)
+    with P.UcLp(lp) as h:
+        sg = h.solve(fixed_iterations=F, trace_attempts=F)
+    assert sg.iterations == so.iterations == F
+    assert np.array_equal(sg.attempts["accepted"], so.attempts["accepted"])
+    assert np.array_equal(sg.attempts["eta_next"][-1000:], so.attempts["eta_next"][-1000:])
+    assert rel_l2(sg.x, so.x) <= 1e-10 and rel_l2(sg.y, so.y) <= 1e-10

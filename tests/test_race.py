@@ -1,0 +1,96 @@
+"""Algorithm 1 of the paper: the racing driver of paper_2607_03627_b200/race.py.
+CPU tests drive its control flow with a stand-in for the GPU handle; the GPU test races the real PDHG solver
+against HiGHS (the stand-in for the paper's barrier solver, which is not available) on UC config 1."""
+import threading
+import time
+from types import SimpleNamespace
+
+import numpy as np
+import pytest
+
+import paper_2607_03627_b200.binding as B
+from paper_2607_03627_b200.race import race
+
+
+class StandInHandle:
+    """Behaves like UcLp for race(): solve() blocks for `seconds` unless cancel() arrives first."""
+
+    def __init__(self, seconds, objective=1.25):
+        self.seconds, self.objective, self._stop, self.cancelled = seconds, objective, threading.Event(), False
+
+    def solve(self, **kw):
+        stopped = self._stop.wait(self.seconds)
+        status = B.CANCELLED if stopped else B.OPTIMAL
+        return SimpleNamespace(status=status, primal_obj=self.objective, iterations=0)
+
+    def cancel(self):
+        self.cancelled = True
+        self._stop.set()
+
+
+def slow_competitor(seconds, value):
+    time.sleep(seconds)
+    return value
+
+
+def delayed_highs(seconds, lp):
+    from helpers import highs
+    time.sleep(seconds)
+    return highs(lp)
+
+
+def test_cpu_wins_and_the_gpu_side_is_cancelled_through_its_hook():
+    h = StandInHandle(seconds=30.0)
+    r = race(h, slow_competitor, (0.2, 7.5), poll_s=0.05)
+    assert r.winner == "cpu" and r.objective == 7.5
+    assert h.cancelled and r.gpu.status == B.CANCELLED
+    assert r.cancel_latency_s is not None and r.cancel_latency_s < 1.0
+    assert r.seconds < 5.0 and r.cpu_seconds is not None
+
+
+def test_gpu_wins_and_the_competitor_process_is_terminated():
+    h = StandInHandle(seconds=0.2, objective=3.0)
+    t0 = time.perf_counter()
+    r = race(h, slow_competitor, (60.0, 9.0), poll_s=0.05)
+    assert r.winner == "gpu_pdhg" and r.objective == 3.0
+    assert not h.cancelled and r.cpu is None and r.cancel_latency_s is None
+    assert time.perf_counter() - t0 < 10.0                 # did not wait for the 60 s competitor
+    assert "competitor terminated" in r.log
+
+
+def test_competitor_failure_does_not_hang_the_race():
+    def broken():
+        raise ValueError("no licence")
+    h = StandInHandle(seconds=0.3, objective=2.0)
+    r = race(h, broken, (), poll_s=0.05)
+    assert r.winner == "gpu_pdhg" and r.objective == 2.0
+
+
+@pytest.mark.gpu
+def test_race_pdhg_against_highs_both_outcomes():
+    """UC config 0 (HiGHS needs ~0.3 s there; on config 1 it needs minutes, see profiles/r01d_race.md)."""
+    import paper_2607_03627_b200 as P
+    from helpers import highs
+    from workloads import uc_config
+    lp = uc_config(0)
+    ref_obj, _, _ = highs(lp)
+    with P.UcLp(lp) as h:
+        h.solve(fixed_iterations=64)                       # warm-up: graph instantiation is not part of the race
+        # default tolerances, both sides at full speed: a genuine race (PDHG ~70 ms, HiGHS ~50-350 ms here)
+        r = race(h, highs, (lp,), competitor_objective=lambda out: out[0], poll_s=0.02)
+        assert r.winner in ("gpu_pdhg", "cpu")
+        assert abs(r.objective - ref_obj) <= 1e-3 * (1.0 + abs(ref_obj))
+        # a competitor held back by 5 s: PDHG converges first and the competitor process is terminated
+        t0 = time.perf_counter()
+        r = race(h, delayed_highs, (5.0, lp), competitor_objective=lambda out: out[0], poll_s=0.02)
+        assert r.winner == "gpu_pdhg" and r.gpu.status == P.OPTIMAL and r.gpu.rel_kkt <= 1e-4 and r.cpu is None
+        assert abs(r.objective - ref_obj) <= 1e-3 * (1.0 + abs(ref_obj)) and time.perf_counter() - t0 < 4.0
+        # an unreachable tolerance: HiGHS wins, the GPU solver is stopped by uc_pdhg_cancel well inside the
+        # paper's 0.5 s poll period
+        r = race(h, highs, (lp,), competitor_objective=lambda out: out[0], poll_s=0.02,
+                 solve_kwargs=dict(eps_rel=0.0, eps_abs=0.0, iter_limit=100_000_000))
+        assert r.winner == "cpu" and r.gpu.status == P.CANCELLED and r.gpu.iterations > 0
+        assert abs(r.objective - ref_obj) <= 1e-9 * (1.0 + abs(ref_obj))
+        assert r.cancel_latency_s < 0.5
+        again = h.solve(fixed_iterations=64)               # the handle survives a race either way
+        assert again.status == P.ITERATION_LIMIT and again.iterations == 64
