@@ -280,22 +280,17 @@ __device__ __forceinline__ void row_dot(const Sell& A, const RowId& r, int lane,
     else long_row<NV>(A, r.lrow, lane, s, gather);
 }
 
-// --------------------------------------------------------------------------- A10 flush before a check
-__global__ void __launch_bounds__(kBlock) k_flush(Vecs V, Ctrl* ctl) {
-    if (ld_flag(&ctl->done) || !ctl->pending) return;
-    const int cur = ctl->cur; const double e = ctl->eta_prev;
-    long long t = (long long)blockIdx.x * kBlock + threadIdx.x;
-    if (t < V.n) V.xsum[t] = V.xsum[t] + e * V.x[cur][t];
-    else if (t - V.n < V.m) { t -= V.n; V.ysum[t] = V.ysum[t] + e * V.y[cur][t]; }
-}
-
 // --------------------------------------------------------------------------- A11 check, dual side
 // per variable j (row of K~'), for z in {current, average}: rho = c - K~'y, lambda, r_d, c.x, bound
 // terms of the dual objective (R9).  partD rows: [rd2_s, rd2_u, pobj, dbound] x {cur, avg}.
-__global__ void __launch_bounds__(kBlock, kCheckMinBlocks) k_check_dual(Sell KT, Vecs V, Ctrl* ctl) {
+// flush != 0 (the periodic check): the pending term of R6 (eta_prev * current iterate, deferred by the attempt
+// kernels) is applied here instead of in a pass of its own: this kernel adds it on the fly to the y-sums it gathers
+// (k_check_primal, which runs next, writes them back) and writes the flushed x-sums of its own rows back.
+__global__ void __launch_bounds__(kBlock, kCheckMinBlocks) k_check_dual(Sell KT, Vecs V, Ctrl* ctl, int flush) {
     __shared__ dd red[8 * 32];
     if (ld_flag(&ctl->done)) return;
     const int cur = ctl->cur;
+    const bool pend = flush && ctl->pending; const double e = ctl->eta_prev;
     const double w = ctl->w; const bool avg = w > 0.0;
     const double* __restrict__ ycur = V.y[cur];
     const double* __restrict__ ysum = V.ysum;
@@ -307,16 +302,19 @@ __global__ void __launch_bounds__(kBlock, kCheckMinBlocks) k_check_dual(Sell KT,
         const RowId r = my_row(KT, vb);
         if (r.row < 0) continue;
         double g[2] = {0.0, 0.0};
-        if (avg) row_dot<2>(KT, r, lane, g, [&](int c, double (&o)[2]) { o[0] = ycur[c]; o[1] = ysum[c] / w; });
+        if (avg) row_dot<2>(KT, r, lane, g, [&](int c, double (&o)[2]) { o[0] = ycur[c]; o[1] = (pend ? ysum[c] + e * o[0] : ysum[c]) / w; });
         else { double g1[1] = {0.0}; row_dot<1>(KT, r, lane, g1, [&](int c, double (&o)[1]) { o[0] = ycur[c]; }); g[0] = g1[0]; }
         if (r.owner) {
             const long long j = r.row;
             const double cj = V.c[j], lj = V.l[j], uj = V.u[j], dc = V.Dc[j];
             const bool lfin = isfinite(lj), ufin = isfinite(uj);
+            const double xc = V.x[cur][j];
+            double xs = V.xsum[j];
+            if (pend) { xs = xs + e * xc; V.xsum[j] = xs; }
 #pragma unroll
             for (int z = 0; z < 2; ++z) {
                 if (z == 1 && !avg) break;
-                const double xj = z ? V.xsum[j] / w : V.x[cur][j];
+                const double xj = z ? xs / w : xc;
                 const double rj = cj - g[z];
                 double lam = 0.0;
                 if (rj > 0.0 && lfin) lam = rj;
@@ -336,10 +334,12 @@ __global__ void __launch_bounds__(kBlock, kCheckMinBlocks) k_check_dual(Sell KT,
 
 // --------------------------------------------------------------------------- A11 check, primal side
 // per row i of K~: a = K~x - q, r_p, q.y (R9).  partP rows: [rp2_s, rp2_u, qy] x {cur, avg}.
-__global__ void __launch_bounds__(kBlock, kCheckMinBlocks) k_check_primal(Sell K, Vecs V, Ctrl* ctl) {
+// flush != 0: the x-sums it gathers were flushed by k_check_dual just before; it flushes the y-sums of its own rows.
+__global__ void __launch_bounds__(kBlock, kCheckMinBlocks) k_check_primal(Sell K, Vecs V, Ctrl* ctl, int flush) {
     __shared__ dd red[6 * 32];
     if (ld_flag(&ctl->done)) return;
     const int cur = ctl->cur;
+    const bool pend = flush && ctl->pending; const double e = ctl->eta_prev;
     const double w = ctl->w; const bool avg = w > 0.0;
     const double* __restrict__ xcur = V.x[cur];
     const double* __restrict__ xsum = V.xsum;
@@ -356,11 +356,14 @@ __global__ void __launch_bounds__(kBlock, kCheckMinBlocks) k_check_primal(Sell K
         if (r.owner) {
             const long long i = r.row;
             const double qi = V.q[i], dr = V.Dr[i]; const int isg = V.isG[i];
+            const double yc = V.y[cur][i];
+            double ys = V.ysum[i];
+            if (pend) { ys = ys + e * yc; V.ysum[i] = ys; }
 #pragma unroll
             for (int z = 0; z < 2; ++z) {
                 if (z == 1 && !avg) break;
                 const double ai = a[z] - qi;
-                const double yi = z ? V.ysum[i] / w : V.y[cur][i];
+                const double yi = z ? ys / w : yc;
                 const double rp = isg ? (ai < 0.0 ? ai : 0.0) : ai;
                 acc[3 * z + 0] = dd_add_d(acc[3 * z + 0], rp * rp);
                 acc[3 * z + 1] = dd_add_d(acc[3 * z + 1], (dr * rp) * (dr * rp));
@@ -437,7 +440,7 @@ __global__ void __launch_bounds__(kFinalBlock) k_check_finalize(Vecs V, Ctrl* ct
     if (mode == kModeReport) { ctl->ret_avg = 0; ctl->status = UC_ITERATION_LIMIT; ctl->done = 1; publish(ctl, Tc); return; }
     if (have_avg) ctl->Tavg = Ta;       // otherwise the previous average terms stay, as in the sequential statement
     ctl->have_avg = have_avg;
-    ctl->pending = 0;                   // k_flush has applied it
+    ctl->pending = 0;                   // the two check kernels have applied it
     const long long k = ctl->k;
     const double omega = ctl->omega;
     const double rk_cur = rel_kkt(ctl, Tc), rk_avg = have_avg ? rel_kkt(ctl, Ta) : INFINITY;

@@ -214,17 +214,17 @@ void launch_primal(uc_lp* lp, cudaStream_t st) { launch_pdl(k_primal, lp->V.grid
 void launch_dual(uc_lp* lp, cudaStream_t st) { launch_pdl(k_dual, lp->V.gridPB, sizeof(DualSmem), st, lp->K, lp->V, lp->ctl); }
 void launch_attempt(uc_lp* lp, cudaStream_t st) { launch_primal(lp, st); launch_dual(lp, st); }
 void launch_kkt(uc_lp* lp, cudaStream_t st, int mode) {
-    k_check_dual<<<lp->V.gridA, kBlock, 0, st>>>(lp->KT, lp->V, lp->ctl);
-    k_check_primal<<<lp->V.gridB, kBlock, 0, st>>>(lp->K, lp->V, lp->ctl);
+    const int flush = mode == kModeCheck;        // the periodic check also applies the pending average term (R6)
+    k_check_dual<<<lp->V.gridA, kBlock, 0, st>>>(lp->KT, lp->V, lp->ctl, flush);
+    k_check_primal<<<lp->V.gridB, kBlock, 0, st>>>(lp->K, lp->V, lp->ctl, flush);
     k_check_finalize<<<1, kFinalBlock, 0, st>>>(lp->V, lp->ctl, mode);
 }
 void launch_check(uc_lp* lp, cudaStream_t st) {
-    k_flush<<<lp->V.gridR, kBlock, 0, st>>>(lp->V, lp->ctl);
     launch_kkt(lp, st, kModeCheck);
     k_restart_vec<<<lp->V.gridR, kBlock, 0, st>>>(lp->V, lp->ctl);
     k_restart_finalize<<<1, kFinalBlock, 0, st>>>(lp->V, lp->ctl);
 }
-constexpr int kCheckLaunches = 6;
+constexpr int kCheckLaunches = 5;
 
 // R2: control block, initial point, KKT components of the restart point z^0 (4 launches); synchronises `st`.
 void start_run(uc_lp* lp, const uc_pdhg_params& prm, cudaStream_t st, long long limit, bool fixed,
