@@ -103,3 +103,27 @@ def test_info_and_launch_count(lp1):
         assert i.bytes_per_attempt > 24 * lp1.nnz
         s = h.solve(fixed_iterations=128)
         assert s.kernel_launches >= 2 * 128 + 2 * 5
+
+
+def test_different_handles_solve_concurrently_on_their_own_streams(lp1):
+    """include/uc_pdhg.h: the call is not re-entrant per handle, but different handles may solve at the same time
+    (the paper's 45 scenarios are independent LPs).  Results must be those of a solve run alone."""
+    with P.UcLp(lp1) as h0:
+        alone = h0.solve(fixed_iterations=640)
+    handles = [P.UcLp(lp1) for _ in range(3)]
+    out = [None] * 3
+
+    def run(i):
+        out[i] = handles[i].solve(fixed_iterations=640)
+
+    try:
+        th = [threading.Thread(target=run, args=(i,)) for i in range(3)]
+        [t.start() for t in th]
+        [t.join(timeout=120) for t in th]
+        assert not any(t.is_alive() for t in th)
+        for s in out:
+            assert s.status == P.ITERATION_LIMIT and s.iterations == 640
+            assert np.array_equal(s.x, alone.x) and np.array_equal(s.y, alone.y)
+    finally:
+        for h in handles:
+            h.close()
