@@ -195,11 +195,6 @@ inline void build_sell(int64_t nrows, const int64_t* ptr, const int32_t* idx, co
     }
 }
 
-struct HostProblem {
-    int64_t m = 0, n = 0, nnz = 0;
-    std::vector<int64_t> perm_r, inv_r, perm_c, inv_c;   // new -> old, old -> new
-    HostSell K, KT;
-};
 
 // Validate the caller's CSR (A0) and return "" or the reason it is rejected.
 inline std::string validate_csr(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, const int32_t* col_idx,
@@ -245,25 +240,37 @@ inline std::string validate_csr(int64_t m, int64_t n, int64_t nnz, const int64_t
     return "";
 }
 
-// A1: explicit transpose (counting sort by column, stable in the row index) + both SELL layouts.
-inline void build_problem(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, const int32_t* col_idx,
-                          const double* val, int64_t window, int64_t long_thr, bool want_src, HostProblem& P) {
+// A1 in three pieces, so that the caller can overlap them (and the upload of K) on two threads:
+//   build_perms  row / column lengths and both permutations (cheap; fixes the slice counts)
+//   build_K      the SELL layout of K
+//   build_KT     explicit transpose (counting sort by column, stable in the row index) + the SELL layout of K'
+struct HostProblem {
+    int64_t m = 0, n = 0, nnz = 0;
+    std::vector<int64_t> perm_r, inv_r, perm_c, inv_c;   // new -> old, old -> new
+    std::vector<int64_t> lenc;                           // entries per column
+    int64_t nshort_r = 0, nshort_c = 0;                  // rows / columns in the sliced parts
+    HostSell K, KT;
+};
+inline void build_perms(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, const int32_t* col_idx,
+                        int64_t window, int64_t long_thr, HostProblem& P) {
     P.m = m; P.n = n; P.nnz = nnz;
-    std::vector<int64_t> lenr((size_t)m), lenc((size_t)n, 0);
+    std::vector<int64_t> lenr((size_t)m);
+    P.lenc.assign((size_t)n, 0);
     for (int64_t i = 0; i < m; ++i) lenr[(size_t)i] = row_ptr[i + 1] - row_ptr[i];
-    for (int64_t p = 0; p < nnz; ++p) lenc[(size_t)col_idx[p]]++;
-    int64_t ms = 0, ns = 0;
-    {
-        std::thread t([&] { build_perm(lenr, window, long_thr, P.perm_r, P.inv_r, ms); });
-        build_perm(lenc, window, long_thr, P.perm_c, P.inv_c, ns);
-        t.join();
-    }
-    std::thread tk([&] { build_sell(m, row_ptr, col_idx, val, nullptr, P.perm_r, ms, P.inv_c, want_src, P.K); });
-    // transpose
+    for (int64_t p = 0; p < nnz; ++p) P.lenc[(size_t)col_idx[p]]++;
+    std::thread t([&] { build_perm(lenr, window, long_thr, P.perm_r, P.inv_r, P.nshort_r); });
+    build_perm(P.lenc, window, long_thr, P.perm_c, P.inv_c, P.nshort_c);
+    t.join();
+}
+inline void build_K(const int64_t* row_ptr, const int32_t* col_idx, const double* val, bool want_src, HostProblem& P) {
+    build_sell(P.m, row_ptr, col_idx, val, nullptr, P.perm_r, P.nshort_r, P.inv_c, want_src, P.K);
+}
+inline void build_KT(const int64_t* row_ptr, const int32_t* col_idx, const double* val, bool want_src, HostProblem& P) {
+    const int64_t m = P.m, n = P.n, nnz = P.nnz;
     std::vector<int64_t> tptr((size_t)n + 1, 0), tsrc(want_src ? (size_t)nnz : 0);
     std::vector<int32_t> tidx((size_t)nnz);
     std::vector<double> tval((size_t)nnz);
-    for (int64_t j = 0; j < n; ++j) tptr[(size_t)j + 1] = tptr[(size_t)j] + lenc[(size_t)j];
+    for (int64_t j = 0; j < n; ++j) tptr[(size_t)j + 1] = tptr[(size_t)j] + P.lenc[(size_t)j];
     // counting sort by column, stable in the row index; each thread owns a range of columns, scans every entry and
     // scatters only its own (its slice of the fill pointers stays in cache)
     parallel_ranges(n, 65536, [&](int64_t jb, int64_t je) {
@@ -277,8 +284,7 @@ inline void build_problem(int64_t m, int64_t n, int64_t nnz, const int64_t* row_
                 if (want_src) tsrc[(size_t)k] = p;
             }
     });
-    build_sell(n, tptr.data(), tidx.data(), tval.data(), want_src ? tsrc.data() : nullptr, P.perm_c, ns, P.inv_r, want_src, P.KT);
-    tk.join();
+    build_sell(n, tptr.data(), tidx.data(), tval.data(), want_src ? tsrc.data() : nullptr, P.perm_c, P.nshort_c, P.inv_r, want_src, P.KT);
 }
 
 

@@ -5,7 +5,10 @@
 #include <chrono>
 #include <cstdio>
 #include <cstring>
+#include <exception>
 #include <limits>
+#include <mutex>
+#include <thread>
 #include <new>
 #include <string>
 #include <vector>
@@ -76,14 +79,18 @@ struct uc_lp {
 
     // every array gets one slice (32 elements) of zeroed slack: the bulk copies of the attempt kernels read
     // whole 32-row segments, and the last slice of the sliced part may be ragged
+    std::mutex alloc_mutex;                // uc_lp_create uploads the two layouts from two threads
     template <class T>
     T* dalloc(size_t count) {
         void* p = nullptr;
         size_t bytes = (count + 32) * sizeof(T);
         cudaError_t e = cudaMalloc(&p, bytes);
         if (e != cudaSuccess) throw CudaFail{e, "cudaMalloc"};
-        allocs.push_back(p);
-        device_bytes += bytes;
+        {
+            std::lock_guard<std::mutex> g(alloc_mutex);
+            allocs.push_back(p);
+            device_bytes += bytes;
+        }
         if (cudaMemset(p, 0, bytes) != cudaSuccess) throw CudaFail{cudaGetLastError(), "cudaMemset"};
         return (T*)p;
     }
@@ -340,24 +347,39 @@ int uc_lp_create(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, cons
         CK(cudaEventCreate(&lp->ev_t0)); CK(cudaEventCreate(&lp->ev_t1));
         cudaStream_t st = lp->own_stream;
 
-        // A0 / A1: layouts (host), upload
+        // A0 / A1: layouts (host), upload.  The K side (layout, schedule, upload) runs on a helper thread while this
+        // thread transposes and builds the K' side.
         HostProblem P;
-        build_problem(m, n, nnz, row_ptr, col_idx, val, opt.sell_window, opt.long_row_threshold, opt.keep_source_map != 0, P);
-        if (P.K.col.size() >= (size_t)1 << 31 || P.KT.col.size() >= (size_t)1 << 31)
-            throw std::bad_alloc();                      // the step descriptors address stored entries / 32 in 26 bits
+        build_perms(m, n, nnz, row_ptr, col_idx, opt.sell_window, opt.long_row_threshold, P);
         int gridPA = 1, gridPB = 1;
         {   // persistent grids of the attempt kernels: kCtasPerSm CTAs per SM, never more CTAs than work; the static
-            // schedule gives slice s to consumer warp s % (grid * kAttWarps)
+            // schedule gives every slice to the consumer warp with the least work so far
             int sms = 0;
             CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
             const int cap = kCtasPerSm * std::max(sms, 1);
-            gridPA = (int)std::max<int64_t>(1, std::min<int64_t>(cap, std::max<int64_t>((P.KT.nslices + kAttWarps - 1) / kAttWarps, P.KT.nlong)));
-            gridPB = (int)std::max<int64_t>(1, std::min<int64_t>(cap, std::max<int64_t>((P.K.nslices + kAttWarps - 1) / kAttWarps, P.K.nlong)));
-            build_schedule(P.KT, (int64_t)gridPA * kAttWarps);
-            build_schedule(P.K, (int64_t)gridPB * kAttWarps);
+            const int64_t sl_kt = (P.nshort_c + 31) / 32, sl_k = (P.nshort_r + 31) / 32;
+            gridPA = (int)std::max<int64_t>(1, std::min<int64_t>(cap, std::max<int64_t>((sl_kt + kAttWarps - 1) / kAttWarps, n - P.nshort_c)));
+            gridPB = (int)std::max<int64_t>(1, std::min<int64_t>(cap, std::max<int64_t>((sl_k + kAttWarps - 1) / kAttWarps, m - P.nshort_r)));
         }
-        lp->K = upload_sell(lp, P.K);
-        lp->KT = upload_sell(lp, P.KT);
+        const bool want_src = opt.keep_source_map != 0;
+        std::exception_ptr k_side_error;
+        std::thread k_side([&] {
+            try {
+                cudaSetDevice(dev);
+                build_K(row_ptr, col_idx, val, want_src, P);
+                if (P.K.col.size() >= (size_t)1 << 31) throw std::bad_alloc();   // step descriptors address entries / 32 in 26 bits
+                build_schedule(P.K, (int64_t)gridPB * kAttWarps);
+                lp->K = upload_sell(lp, P.K);
+            } catch (...) { k_side_error = std::current_exception(); }
+        });
+        try {
+            build_KT(row_ptr, col_idx, val, want_src, P);
+            if (P.KT.col.size() >= (size_t)1 << 31) throw std::bad_alloc();
+            build_schedule(P.KT, (int64_t)gridPA * kAttWarps);
+            lp->KT = upload_sell(lp, P.KT);
+        } catch (...) { k_side.join(); throw; }
+        k_side.join();
+        if (k_side_error) std::rethrow_exception(k_side_error);
         lp->k_slots = (int64_t)P.K.col.size(); lp->kt_slots = (int64_t)P.KT.col.size();
         lp->k_long_nnz = (int64_t)P.K.lcol.size(); lp->kt_long_nnz = (int64_t)P.KT.lcol.size();
         lp->perm_r = (long long*)lp->upload(P.perm_r);
