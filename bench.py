@@ -43,7 +43,7 @@ def algorithmic_bytes(m, n, nnz):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the attempt kernels on config 3, from the one
 # `ncu --set full` capture summarised in profiles/r01d_summary.md (cold L2 per replay; bytes)
-NCU_TRAFFIC_CONFIG3 = {"k_primal": 185.05e6 + 13.60e6, "k_dual": 161.41e6 + 4.67e6, "source": "profiles/r01d_summary.md"}
+NCU_TRAFFIC_CONFIG3 = {"k_primal": 185.04e6 + 14.06e6, "k_dual": 161.37e6 + 4.17e6, "source": "profiles/r01d_summary.md"}
 
 
 def load_peaks():
