@@ -187,6 +187,14 @@ int uc_lp_get_scaled_values(uc_lp* lp, int32_t from_transpose, double* val_out);
    solver's own SpMV kernels; HOST in/out, original order.  Test hook for the adjoint identity. */
 int uc_lp_spmv(uc_lp* lp, int32_t transpose, const double* v, double* out);
 
+/* Host-only self-check of ingest step A1 (no GPU needed): builds the row / column permutations, the explicit
+   transpose, both SELL-32 layouts and both attempt schedules (for `sched_warps` consumer warps) exactly as
+   uc_lp_create does, and verifies them entry by entry against the caller's CSR: stored entries are the caller's, in
+   the caller's order (K' rows in ascending caller row index), padding is (0, 0.0), every slice is scheduled exactly
+   once as consecutive chunks.  Returns UC_OK, or UC_ERR_INVALID with the violated property in uc_last_error(). */
+int uc_host_layout_selftest(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, const int32_t* col_idx, const double* val,
+                            int32_t sell_window, int32_t long_row_threshold, int32_t sched_warps);
+
 /* Host evaluation of the double-double log / exp that the primal-weight update (R11) runs on the
    device (same source, csrc/uc_dd.cuh).  Test hooks: no GPU needed. */
 double uc_host_log_rounded(double a);

@@ -62,7 +62,7 @@ CHECK_DTYPE = np.dtype([("k", "i8"), ("restart_kind", "i4"), ("candidate", "i4")
 EXPORTS = ["uc_lp_default_options", "uc_lp_create", "uc_lp_update_bounds", "uc_lp_destroy",
            "uc_pdhg_default_params", "uc_pdhg_solve", "uc_pdhg_solve_device", "uc_pdhg_cancel", "uc_pdhg_time_kernels",
            "uc_lp_get_info", "uc_lp_get_scaling", "uc_lp_get_scaled_values", "uc_lp_spmv", "uc_last_error",
-           "uc_host_log_rounded", "uc_host_exp_rounded"]
+           "uc_host_log_rounded", "uc_host_exp_rounded", "uc_host_layout_selftest"]
 
 _lib = None
 
@@ -96,6 +96,8 @@ def load_library(build_if_missing: bool = True):
     lib.uc_pdhg_solve.argtypes = [C.c_void_p] * 5
     lib.uc_pdhg_solve_device.argtypes = [C.c_void_p] * 5
     lib.uc_pdhg_time_kernels.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
+    lib.uc_host_layout_selftest.argtypes = [C.c_int64, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p,
+                                            C.c_int32, C.c_int32, C.c_int32]
     lib.uc_lp_get_info.argtypes = [C.c_void_p] * 2
     lib.uc_lp_get_scaling.argtypes = [C.c_void_p] * 3
     lib.uc_lp_get_scaled_values.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
@@ -107,6 +109,15 @@ def load_library(build_if_missing: bool = True):
 def _check(rc):
     if rc != 0:
         raise UcError(rc, load_library().uc_last_error().decode())
+
+
+def host_layout_selftest(lp, sell_window=4096, long_row_threshold=32, sched_warps=148 * 15) -> None:
+    """uc_host_layout_selftest on a workloads.LP; raises UcError with the violated property."""
+    lib = load_library()
+    rp = np.ascontiguousarray(lp.row_ptr, dtype=np.int64); ci = np.ascontiguousarray(lp.col_idx, dtype=np.int32)
+    va = np.ascontiguousarray(lp.val, dtype=np.float64)
+    _check(lib.uc_host_layout_selftest(int(lp.m), int(lp.n), int(lp.nnz), C.c_void_p(rp.ctypes.data), C.c_void_p(ci.ctypes.data),
+                                       C.c_void_p(va.ctypes.data), int(sell_window), int(long_row_threshold), int(sched_warps)))
 
 
 def default_options(**kw) -> Options:

@@ -298,6 +298,127 @@ extern "C" {
 const char* uc_last_error(void) { return g_err.c_str(); }
 
 
+// Host-only check of A0/A1 (no device): builds the permutations, both SELL-32 layouts and both attempt schedules
+// exactly as uc_lp_create does and verifies them against the caller's CSR.  Returns UC_OK or UC_ERR_INVALID with
+// the first violated property in uc_last_error().
+int uc_host_layout_selftest(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, const int32_t* col_idx, const double* val,
+                            int32_t sell_window, int32_t long_row_threshold, int32_t sched_warps) {
+    if (m < 0 || n < 0 || nnz < 0 || !row_ptr || sell_window < 32 || long_row_threshold < 1 || sched_warps < 1)
+        return fail(UC_ERR_INVALID, "bad argument");
+    HostProblem P;
+    build_perms(m, n, nnz, row_ptr, col_idx, sell_window, long_row_threshold, P);
+    build_K(row_ptr, col_idx, val, true, P);
+    build_KT(row_ptr, col_idx, val, true, P);
+    build_schedule(P.K, sched_warps);
+    build_schedule(P.KT, sched_warps);
+    auto bad = [&](const std::string& what) { return fail(UC_ERR_INVALID, what); };
+    // ---- permutations: bijections, rows with <= threshold entries first, the others last in the caller's order
+    auto check_perm = [&](const std::vector<int64_t>& perm, const std::vector<int64_t>& inv, int64_t N, int64_t nshort,
+                          const std::vector<int64_t>& len) -> const char* {
+        if ((int64_t)perm.size() != N || (int64_t)inv.size() != N) return "permutation size";
+        std::vector<char> seen((size_t)N, 0);
+        for (int64_t k = 0; k < N; ++k) {
+            const int64_t o = perm[(size_t)k];
+            if (o < 0 || o >= N || seen[(size_t)o]) return "not a permutation";
+            seen[(size_t)o] = 1;
+            if (inv[(size_t)o] != k) return "inverse permutation";
+            if ((k < nshort) != (len[(size_t)o] <= long_row_threshold)) return "short / long split";
+            if (k > nshort && perm[(size_t)k - 1] > o) return "long rows out of order";
+        }
+        return nullptr;
+    };
+    std::vector<int64_t> lenr((size_t)m);
+    for (int64_t i = 0; i < m; ++i) lenr[(size_t)i] = row_ptr[i + 1] - row_ptr[i];
+    if (const char* w = check_perm(P.perm_r, P.inv_r, m, P.nshort_r, lenr)) return bad(std::string("rows: ") + w);
+    if (const char* w = check_perm(P.perm_c, P.inv_c, n, P.nshort_c, P.lenc)) return bad(std::string("columns: ") + w);
+    // ---- expected K' rows: for column j the entries (i, K_ij) in ascending caller row order (what the sequential
+    // statement's column scatter produces)
+    std::vector<std::vector<std::pair<int64_t, int64_t>>> cols((size_t)n);       // (row, CSR position)
+    for (int64_t i = 0; i < m; ++i)
+        for (int64_t p = row_ptr[i]; p < row_ptr[i + 1]; ++p) cols[(size_t)col_idx[p]].push_back({i, p});
+    // ---- layouts: every stored entry is the caller's entry, in the caller's order, relabelled; padding is (0, 0.0)
+    auto check_sell = [&](const HostSell& S, bool transposed) -> std::string {
+        const std::vector<int64_t>& perm = transposed ? P.perm_c : P.perm_r;
+        const std::vector<int64_t>& inv_other = transposed ? P.inv_r : P.inv_c;
+        const int64_t N = transposed ? n : m;
+        if (S.nrows != N || S.nshort + S.nlong != N || S.nslices != (S.nshort + 31) / 32) return "counts";
+        auto row_len = [&](int64_t o) { return transposed ? (int64_t)cols[(size_t)o].size() : row_ptr[o + 1] - row_ptr[o]; };
+        auto entry = [&](int64_t o, int64_t t, int64_t& c_new, double& v, int64_t& pos) {
+            if (transposed) { pos = cols[(size_t)o][(size_t)t].second; c_new = inv_other[(size_t)cols[(size_t)o][(size_t)t].first]; }
+            else { pos = row_ptr[o] + t; c_new = inv_other[(size_t)col_idx[pos]]; }
+            v = val[pos];
+        };
+        for (int64_t s = 0; s < S.nslices; ++s) {
+            int64_t w = 0;
+            for (int64_t r = 32 * s; r < std::min<int64_t>(32 * s + 32, S.nshort); ++r) w = std::max(w, row_len(perm[(size_t)r]));
+            if (S.slice_ptr[(size_t)s + 1] - S.slice_ptr[(size_t)s] != 32 * w) return "slice width";
+            for (int64_t lane = 0; lane < 32; ++lane) {
+                const int64_t r = 32 * s + lane;
+                const int64_t len = r < S.nshort ? row_len(perm[(size_t)r]) : 0;
+                for (int64_t t = 0; t < w; ++t) {
+                    const size_t k = (size_t)(S.slice_ptr[(size_t)s] + 32 * t + lane);
+                    if (t < len) {
+                        int64_t c_new, pos; double v;
+                        entry(perm[(size_t)r], t, c_new, v, pos);
+                        if (S.col[k] != (int32_t)c_new || std::memcmp(&S.val[k], &v, sizeof v) != 0 || S.src[k] != pos) return "stored entry";
+                    } else if (S.col[k] != 0 || S.val[k] != 0.0 || S.src[k] != -1) return "padding slot";
+                }
+            }
+        }
+        for (int64_t r = 0; r < S.nlong; ++r) {
+            const int64_t o = perm[(size_t)(S.nshort + r)];
+            if (S.lptr[(size_t)r + 1] - S.lptr[(size_t)r] != row_len(o)) return "long row length";
+            for (int64_t t = 0; t < row_len(o); ++t) {
+                int64_t c_new, pos; double v;
+                entry(o, t, c_new, v, pos);
+                const size_t k = (size_t)(S.lptr[(size_t)r] + t);
+                if (S.lcol[k] != (int32_t)c_new || std::memcmp(&S.lval[k], &v, sizeof v) != 0 || S.lsrc[k] != pos) return "long row entry";
+            }
+        }
+        // ---- schedule: every slice exactly once, as consecutive chunks of one warp, flags and offsets right
+        const int64_t W = S.sched_warps, J = S.steps_per_warp;
+        if ((int64_t)S.steps.size() != W * J) return "schedule size";
+        std::vector<int> done((size_t)S.nslices, 0);
+        for (int64_t wq = 0; wq < W; ++wq) {
+            bool ended = false; int64_t prev_slice = -1;
+            for (int64_t j = 0; j < J; ) {
+                const StepDesc d = S.steps[(size_t)(j * W + wq)];
+                const uint32_t info = d.w0 >> 26;
+                if (ended) { if (d.w0 != 0 || d.row0 != 0) return "step after the end marker"; ++j; continue; }
+                if (info & kStepEnd) { if ((info & 31) != 0) return "end marker carries work"; ended = true; ++j; continue; }
+                if (!(info & kStepFirst) || d.row0 % 32) return "slice does not start with its first chunk";
+                const int64_t sl = d.row0 / 32;
+                if (sl < 0 || sl >= S.nslices || done[(size_t)sl]++) return "slice scheduled twice or out of range";
+                if (sl <= prev_slice) return "a warp's slices are not ascending";
+                prev_slice = sl;
+                const int64_t wd = (S.slice_ptr[(size_t)sl + 1] - S.slice_ptr[(size_t)sl]) / 32;
+                const int64_t nch = std::max<int64_t>(1, (wd + kChunkT - 1) / kChunkT);
+                for (int64_t c = 0; c < nch; ++c, ++j) {
+                    if (j >= J) return "slice cut off by the end of the schedule";
+                    const StepDesc e = S.steps[(size_t)(j * W + wq)];
+                    const uint32_t ei = e.w0 >> 26;
+                    const int64_t nt = std::max<int64_t>(0, std::min<int64_t>(kChunkT, wd - kChunkT * c));
+                    if (e.row0 != d.row0 || (int64_t)(ei & 7) != nt || ((ei & kStepFirst) != 0) != (c == 0) ||
+                        ((ei & kStepLast) != 0) != (c == nch - 1) || (ei & kStepEnd) ||
+                        ((int64_t)(e.w0 & 0x3ffffffu) << 5) != S.slice_ptr[(size_t)sl] + 32 * kChunkT * c)
+                        return "chunk descriptor";
+                }
+            }
+            if (!ended && J > 0) {                       // a warp without end marker must own the full J steps
+                const uint32_t li = S.steps[(size_t)((J - 1) * W + wq)].w0 >> 26;
+                if (!(li & kStepLast)) return "last step of a full warp is not a last chunk";
+            }
+        }
+        for (int64_t sl = 0; sl < S.nslices; ++sl) if (done[(size_t)sl] != 1) return "slice not scheduled";
+        return "";
+    };
+    std::string w = check_sell(P.K, false);
+    if (!w.empty()) return bad("K layout: " + w);
+    w = check_sell(P.KT, true);
+    if (!w.empty()) return bad("K' layout: " + w);
+    return UC_OK;
+}
+
 double uc_host_log_rounded(double a) { return log_rounded(a); }
 double uc_host_exp_rounded(double x) { return exp_rounded(x); }
 
