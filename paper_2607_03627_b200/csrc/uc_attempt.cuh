@@ -31,8 +31,8 @@
 // L2 policy: streamed-once data is loaded (cp.async.cg, L1 bypass) and stored evict_first; the gathered vectors
 // (y', {xbar, dx}) are stored evict_last so that the gathers of the NEXT kernel hit in the 126 MB L2.
 // Every thread keeps its double-double partial sums in registers across all its steps; there is ONE block
-// reduction per kernel, then one partial per CTA, and the last CTA to finish (ticket) adds the <= 2 * #SM
-// partials.
+// reduction per kernel, then one partial per CTA; warp 0 of the last CTA to finish (ticket) adds the <= #SM
+// partials with shuffles only and runs the step rule on scalars it fetched while the kernel started.
 //
 // Arithmetic is unchanged from the sequential statement: row sums left to right in CSR order, multiply
 // and add rounded separately (-fmad=false), long reductions in double-double (order-independent once
@@ -111,7 +111,6 @@ template <int NVEC, bool BYTEVEC, class GT>
 struct SmemT {
     WarpRing<NVEC, BYTEVEC, GT> w[kAttWarps];
     dd red[2 * 32];
-    int is_last;
 };
 using PrimalSmem = SmemT<5, false, double>;   // x, c, l, u, xsum ; gathers y
 using DualSmem = SmemT<3, true, double2>;     // y, q, ysum + isG ; gathers {xbar, dx}

@@ -149,18 +149,6 @@ __device__ __forceinline__ void block_sum_dd(dd (&v)[NV], dd* red) {
     __syncthreads();
 }
 
-// true in every thread of the block that finishes last (after all partials are globally visible)
-__device__ __forceinline__ bool last_block_done(unsigned int* ticket) {
-    __shared__ int is_last;
-    if (threadIdx.x == 0) {
-        __threadfence();
-        unsigned int t = atomicAdd(ticket, 1u);
-        is_last = (t == gridDim.x - 1);
-    }
-    __syncthreads();
-    return is_last != 0;
-}
-
 // double-double sums of NV partial arrays (part + q * stride, `count` entries each) by one block, in one pass;
 // results valid in thread 0
 template <int NV>
@@ -175,11 +163,6 @@ __device__ __forceinline__ void final_sums(const dd* part, long long stride, int
         }
     }
     block_sum_dd<NV>(v, red);
-}
-__device__ __forceinline__ dd final_sum(const dd* part, int count, dd* red) {
-    dd v[1];
-    final_sums<1>(part, 0, count, v, red);
-    return v[0];
 }
 
 // --------------------------------------------------------------------------- row ownership
