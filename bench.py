@@ -154,6 +154,54 @@ def aggregate(local_seconds, local_units, dist=None, device=None):
     return float(t.item()), float(u.item())
 
 
+def all_configs_table(handles=(1, 2, 3)):
+    """--all-configs: one markdown table over BASELINE.json's configs (UC 0-3, roofline sweep seeds 10-13): attempts/s of
+    `uc_pdhg_solve_device` with fixed attempts (CUDA-event loop time), and the aggregate rate of concurrent handles
+    on the latency-bound config 1.  Reporting only: the bench line of the contract is the default run."""
+    import threading
+    import torch
+    import paper_2607_03627_b200 as P
+    from workloads import sweep_config, uc_config
+    peak, _ = load_peaks()
+    st = torch.cuda.Stream()
+    print("| workload | m | n | nnz | us/attempt (in graph, checks incl.) | attempts/s | algorithmic MB/attempt | GB/s | % of measured peak | device MB | create ms |")
+    print("|---|---|---|---|---|---|---|---|---|---|---|")
+    cases = [(f"UC config {c}", (lambda c=c: uc_config(c)), 2048) for c in (0, 1, 2, 3)]
+    cases += [(f"config 4, seed {s_}", (lambda s_=s_: sweep_config(s_)), 200 if s_ < 13 else 64) for s_ in (10, 11, 12, 13)]
+    for name, make, attempts in cases:
+        lp = make()
+        t = time.perf_counter(); h = P.UcLp(lp, device=0); tc = time.perf_counter() - t
+        x = torch.empty(lp.n, dtype=torch.float64, device="cuda"); y = torch.empty(lp.m, dtype=torch.float64, device="cuda")
+        for _ in range(2):
+            r = h.solve_device(x, y, fixed_iterations=attempts, stream=st.cuda_stream)
+        us = r.loop_seconds * 1e6 / attempts
+        bp, bd = algorithmic_bytes(lp.m, lp.n, lp.nnz)
+        print(f"| {name} | {lp.m} | {lp.n} | {lp.nnz} | {us:.2f} | {1e6 / us:.0f} | {(bp + bd) / 1e6:.1f} | {(bp + bd) / us / 1e3:.0f} | "
+              f"{(bp + bd) / us / 1e3 / peak * 100:.1f} | {h.info().device_bytes / 1e6:.0f} | {tc * 1e3:.0f} |", flush=True)
+        h.close()
+    print()
+    print("| config | concurrent handles (one thread and one stream each) | aggregate attempts/s | results identical |")
+    print("|---|---|---|---|")
+    lp = uc_config(1)
+    for nh in handles:
+        hs = [P.UcLp(lp, device=0) for _ in range(nh)]
+        sts = [torch.cuda.Stream() for _ in range(nh)]
+        xs = [torch.empty(lp.n, dtype=torch.float64, device="cuda") for _ in range(nh)]
+        ys = [torch.empty(lp.m, dtype=torch.float64, device="cuda") for _ in range(nh)]
+
+        def run(i):
+            hs[i].solve_device(xs[i], ys[i], fixed_iterations=2048, stream=sts[i].cuda_stream)
+        for _ in range(2):
+            th = [threading.Thread(target=run, args=(i,)) for i in range(nh)]
+            torch.cuda.synchronize(); t = time.perf_counter()
+            [t_.start() for t_ in th]; [t_.join() for t_ in th]
+            torch.cuda.synchronize(); dt = time.perf_counter() - t
+        same = all(torch.equal(xs[0], xs[i]) for i in range(1, nh))
+        print(f"| 1 | {nh} | {nh * 2048 / dt:.0f} | {same} |", flush=True)
+        for h in hs:
+            h.close()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -165,7 +213,10 @@ def main():
     ap.add_argument("--ref-attempts", type=int, default=20)
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--all-configs", action="store_true", help="print the table over all configs instead of the bench line")
     args = ap.parse_args()
+    if args.all_configs:
+        return all_configs_table()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
     rank = int(os.environ.get("RANK", "0"))

@@ -109,3 +109,49 @@ def race(handle: "_b.UcLp", competitor: Callable[..., Any], competitor_args: tup
     res.gpu = box.get("sol")
     res.gpu_seconds = box.get("t")
     return res
+
+
+def highs_competitor(lp):
+    """Stand-in for the paper's CPU barrier solver: HiGHS through scipy (optional dependency).  Returns the optimal
+    objective of min c'x s.t. Ax {=,>=} b, l <= x <= u."""
+    import numpy as np
+    import scipy.sparse as sp
+    from scipy.optimize import linprog
+    A = sp.csr_matrix((lp.val, lp.col_idx, lp.row_ptr), shape=(lp.m, lp.n))
+    E = np.asarray(lp.sense) == ord("E")
+    G = ~E
+    bounds = [(None if np.isinf(a) else a, None if np.isinf(b) else b) for a, b in zip(lp.l, lp.u)]
+    kw = {}
+    if G.any():
+        kw.update(A_ub=-A[G], b_ub=-lp.b[G])
+    if E.any():
+        kw.update(A_eq=A[E], b_eq=lp.b[E])
+    r = linprog(lp.c, bounds=bounds, method="highs", **kw)
+    if r.status != 0:
+        raise RuntimeError(r.message)
+    return float(r.fun)
+
+
+def _main():
+    """python -m paper_2607_03627_b200.race --configs 0 1 [--poll 0.05] [--alone-limit-s 600]: one table row per UC config."""
+    import argparse
+    from workloads import uc_config
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--configs", type=int, nargs="+", default=[0, 1])
+    ap.add_argument("--poll", type=float, default=0.05)
+    args = ap.parse_args()
+    print("| config | winner | race s | GPU PDHG alone s (attempts) | HiGHS alone s | objective | cancel latency ms |")
+    print("|---|---|---|---|---|---|---|")
+    for c in args.configs:
+        lp = uc_config(c)
+        with _b.UcLp(lp) as h:
+            h.solve(fixed_iterations=64)                  # warm-up: graph instantiation is not part of the race
+            r = race(h, highs_competitor, (lp,), poll_s=args.poll)
+            t = time.perf_counter(); s = h.solve(); tg = time.perf_counter() - t
+        t = time.perf_counter(); highs_competitor(lp); tc = time.perf_counter() - t
+        lat = "-" if r.cancel_latency_s is None else f"{1e3 * r.cancel_latency_s:.1f}"
+        print(f"| {c} | {r.winner} | {r.seconds:.2f} | {tg:.3f} ({s.iterations}) | {tc:.2f} | {r.objective:.4f} | {lat} |", flush=True)
+
+
+if __name__ == "__main__":
+    _main()
