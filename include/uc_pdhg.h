@@ -148,9 +148,14 @@ int uc_pdhg_solve(uc_lp* lp, const uc_pdhg_params* params, double* x_out, double
 int uc_pdhg_solve_device(uc_lp* lp, const uc_pdhg_params* params, double* x_out_device, double* y_out_device,
                          uc_pdhg_result* result);
 
-/* Sticky cancel flag, any thread, idempotent.  A solve that finds it set -- at entry or at any
-   check -- returns UC_CANCELLED and clears it, so a cancel that lands just before the solve starts
-   is not lost (the race of Algorithm 1). */
+/* Cancel, any thread, idempotent (Algorithm 1: "Terminate the other solver").
+   - A solve is in flight on the handle: THAT solve returns UC_CANCELLED at its next check (within one check
+     period).  The request is scoped to it: if the solve was already past its last check and returns with
+     another status, the request is dropped -- it never leaks into a later solve on the handle.
+   - The handle is idle: the request is kept for the NEXT solve, which returns UC_CANCELLED at entry with
+     iterations = 0 and x_out / y_out untouched -- so a cancel that lands just before the solve starts is not
+     lost (the race of Algorithm 1).
+   A cancel that races with the very start of a solve takes one of these two routes; both stop that solve. */
 int uc_pdhg_cancel(uc_lp* lp);
 
 /* Measurement hook: from the initial point, run `attempts` attempts as plain stream

@@ -99,13 +99,18 @@ class Solution:
     avg_w: float
     Dr: np.ndarray
     Dc: np.ndarray
+    check_x: np.ndarray | None = None      # [checks, n] scaled current iterate as each check saw it
+    check_y: np.ndarray | None = None
+    check_avg_x: np.ndarray | None = None  # [checks, n] scaled average at each check (current iterate if w = 0)
+    check_avg_y: np.ndarray | None = None
+    check_w: np.ndarray | None = None      # [checks] weight sum w at each check
 
 
 def _csr(lp):
     return (C.c_int64(lp.m), C.c_int64(lp.n), _p(lp.row_ptr, C.c_int64), _p(lp.col_idx, C.c_int32), _p(lp.val))
 
 
-def solve(lp, x0=None, y0=None, trace_attempts=0, trace_checks=4096, dump=0, **params) -> Solution:
+def solve(lp, x0=None, y0=None, trace_attempts=0, trace_checks=4096, dump=0, dump_checks=0, **params) -> Solution:
     """Run the oracle on `lp` (a workloads.LP).  Keyword params override oracle_default_params."""
     prm = default_params(**params)
     m, n = lp.m, lp.n
@@ -117,6 +122,11 @@ def solve(lp, x0=None, y0=None, trace_attempts=0, trace_checks=4096, dump=0, **p
     dy = np.zeros((dump, m)) if dump else None
     ax = np.zeros(n); ay = np.zeros(m); aw = C.c_double(0.0)
     Dr = np.zeros(m); Dc = np.zeros(n)
+    cx = np.zeros((dump_checks, n)) if dump_checks else None
+    cy = np.zeros((dump_checks, m)) if dump_checks else None
+    cax = np.zeros((dump_checks, n)) if dump_checks else None
+    cay = np.zeros((dump_checks, m)) if dump_checks else None
+    cw = np.zeros(dump_checks) if dump_checks else None
     res = Result()
     x0 = None if x0 is None else np.ascontiguousarray(x0, dtype=np.float64)
     y0 = None if y0 is None else np.ascontiguousarray(y0, dtype=np.float64)
@@ -124,7 +134,8 @@ def solve(lp, x0=None, y0=None, trace_attempts=0, trace_checks=4096, dump=0, **p
                                  C.byref(prm), _p(x0), _p(y0), _p(x), _p(y), C.byref(res),
                                  C.c_void_p(att.ctypes.data), C.c_int64(trace_attempts), C.byref(na),
                                  C.c_void_p(chk.ctypes.data), C.c_int64(trace_checks), C.byref(nc),
-                                 _p(dx), _p(dy), C.c_int64(dump), _p(ax), _p(ay), C.byref(aw), _p(Dr), _p(Dc))
+                                 _p(dx), _p(dy), C.c_int64(dump), _p(ax), _p(ay), C.byref(aw), _p(Dr), _p(Dc),
+                                 _p(cx), _p(cy), _p(cax), _p(cay), _p(cw), C.c_int64(dump_checks))
     if rc != 0:
         raise ValueError(f"oracle_pdhg_solve returned {rc}")
     return Solution(x=x, y=y, status=res.status, returned_average=res.returned_average,
@@ -133,7 +144,12 @@ def solve(lp, x0=None, y0=None, trace_attempts=0, trace_checks=4096, dump=0, **p
                     rel_gap=res.rel_gap, primal_obj=res.primal_obj, dual_obj=res.dual_obj, eta=res.eta,
                     omega=res.omega, attempts=att[:min(na.value, trace_attempts)],
                     checks=chk[:min(nc.value, trace_checks)], dump_x=dx, dump_y=dy,
-                    avg_x=ax, avg_y=ay, avg_w=aw.value, Dr=Dr, Dc=Dc)
+                    avg_x=ax, avg_y=ay, avg_w=aw.value, Dr=Dr, Dc=Dc,
+                    check_x=None if cx is None else cx[:min(nc.value, dump_checks)],
+                    check_y=None if cy is None else cy[:min(nc.value, dump_checks)],
+                    check_avg_x=None if cax is None else cax[:min(nc.value, dump_checks)],
+                    check_avg_y=None if cay is None else cay[:min(nc.value, dump_checks)],
+                    check_w=None if cw is None else cw[:min(nc.value, dump_checks)])
 
 
 def precondition(lp, ruiz_iters=10, pc_alpha=1.0):

@@ -13,13 +13,15 @@
  * may build, load or call this file.  It shares no code, header, table or helper with
  * paper_2607_03627_b200/ (the CUDA path) and neither includes the other.
  *
- * Pins (tests/test_oracle_*.py): brute-force vertex enumeration (n <= 8), HiGHS objective,
- * box-only and merit-order closed forms, the worked 1x1 step example and the worked 2x2
- * preconditioner example of SURVEY.md 8(c) (tests/golden/), sigma_max <= 1 after
- * Pock-Chambolle, Fejer monotonicity with a frozen step, explicit weighted averages,
- * KKT / complementary slackness.  The restart rule and the primal-weight update (R10, R11)
- * have no external pin beyond invariants and end-to-end convergence: "parity unpinned"
- * for those two decisions (also stated in DESIGN.md).
+ * Pins (tests/test_oracle_pins.py; DESIGN.md section 4 lists which reading each one covers): brute-force vertex
+ * enumeration (n <= 8), HiGHS objective, box-only and merit-order closed forms, the worked 1x1 step example and
+ * the worked 2x2 preconditioner example of SURVEY.md 8(c) (tests/golden/), sigma_max <= 1 after Pock-Chambolle,
+ * Fejer monotonicity with a frozen step, explicit weighted averages, KKT / complementary slackness.  The restart
+ * rule and the primal-weight update (R10, R11) are pinned by the worked restart example
+ * (tests/golden/restart_1x1.txt, derived by hand in DESIGN.md: all three restart kinds, restarts to the average,
+ * a moving primal weight) and by an independent dense-numpy recomputation of every decision and of the closed
+ * form omega_new = (Dy/Dx)^theta omega^(1-theta) from the iterates dumped at each check (tests/helpers.py
+ * restart_replay).  Every function of this file has a pin.
  *
  * Numerics: IEEE fp64, round to nearest, compiled with -ffp-contract=off.  SpMV row sums run
  * in CSR order; every long reduction (norm, dot, objective) is Neumaier-compensated so that
@@ -252,7 +254,13 @@ static double* dalloc(int64_t k) { return (double*)calloc((size_t)(k > 0 ? k : 1
  * att[att_cap], chk[chk_cap] (counts written to *n_att, *n_chk; records beyond capacity are
  * dropped); dump_x[dump_cap*n], dump_y[dump_cap*m]: the SCALED current iterate after each of
  * the first dump_cap attempts; avg_x[n], avg_y[m], *avg_w: final scaled weighted sums / w.
- * Dr_out[m], Dc_out[n] (nullable): the scalings used.  Returns 0, or -1 on bad arguments.
+ * Dr_out[m], Dc_out[n] (nullable): the scalings used.
+ * Check dumps (nullable, TRACE ONLY -- they read the state, they never change it): for each of the first
+ * cdump_cap checks, cdump_x[i*n..], cdump_y[i*m..] = the SCALED current iterate as the check sees it (before any
+ * restart is applied), cdump_ax / cdump_ay = the SCALED average x_sum/w, y_sum/w (the current iterate if w = 0),
+ * cdump_w[i] = w.  They let a test recompute every restart decision and primal-weight update (R10, R11) from
+ * the iterates with its own algebra.
+ * Returns 0, or -1 on bad arguments.
  */
 int oracle_pdhg_solve(int64_t m, int64_t n, const int64_t* row_ptr, const int32_t* col, const double* val,
                       const unsigned char* sense, const double* b, const double* c, const double* l,
@@ -262,7 +270,9 @@ int oracle_pdhg_solve(int64_t m, int64_t n, const int64_t* row_ptr, const int32_
                       oracle_check* chk, int64_t chk_cap, int64_t* n_chk,
                       double* dump_x, double* dump_y, int64_t dump_cap,
                       double* avg_x, double* avg_y, double* avg_w,
-                      double* Dr_out, double* Dc_out) {
+                      double* Dr_out, double* Dc_out,
+                      double* cdump_x, double* cdump_y, double* cdump_ax, double* cdump_ay, double* cdump_w,
+                      int64_t cdump_cap) {
     if (m < 0 || n < 0 || !prm || !res || prm->check_every <= 0) return -1;
     int64_t nnz = row_ptr[m];
     sprob P; memset(&P, 0, sizeof P);
@@ -366,6 +376,13 @@ int oracle_pdhg_solve(int64_t m, int64_t n, const int64_t* row_ptr, const int32_
             for (int64_t j = 0; j < n; ++j) xavg[j] = xsum[j] / w;
             for (int64_t i = 0; i < m; ++i) yavg[i] = ysum[i] / w;
             kkt_eval(&P, xavg, yavg, sa, srho, &Tavg);
+        }
+        if (nc < cdump_cap) {                                  /* trace only */
+            if (cdump_x) memcpy(cdump_x + nc * n, x, sizeof(double) * (size_t)n);
+            if (cdump_y) memcpy(cdump_y + nc * m, y, sizeof(double) * (size_t)m);
+            if (cdump_ax) memcpy(cdump_ax + nc * n, have_avg ? xavg : x, sizeof(double) * (size_t)n);
+            if (cdump_ay) memcpy(cdump_ay + nc * m, have_avg ? yavg : y, sizeof(double) * (size_t)m);
+            if (cdump_w) cdump_w[nc] = w;
         }
         double rk_cur = rel_kkt(&P, &Tcur), rk_avg = have_avg ? rel_kkt(&P, &Tavg) : INFINITY;
         if (!isfinite(rk_cur)) { status = ORACLE_NUMERICAL_ERROR; break; }

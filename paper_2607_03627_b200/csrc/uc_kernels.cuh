@@ -53,7 +53,8 @@ struct Ctrl {
     const double2* powtab;     // [limit] entry k-1 = {(k+1)^-0.6, (k+1)^-0.3} for attempt k (R5)
     uc_attempt_record* att; long long att_cap;
     uc_check_record* chk; long long chk_cap;
-    const int* host_stop;      // mapped host flag: 0 none, UC_CANCELLED or UC_TIME_LIMIT requested
+    const int* host_stop;      // mapped host flag: (solve generation << 3) | UC_CANCELLED or UC_TIME_LIMIT; 0 = none
+    int gen, pad4;             // generation of the solve in flight: a stop request of another generation is stale
     HostStatus* host_status;   // mapped host record
 };
 
@@ -437,8 +438,8 @@ __global__ void __launch_bounds__(kFinalBlock) k_check_finalize(Vecs V, Ctrl* ct
         else if (converged(ctl, Tc)) { status = UC_OPTIMAL; ret_avg = 0; }
     }
     if (status < 0) {
-        const int stop = *(const volatile int*)ctl->host_stop;    // cancel / time limit from the host
-        if (stop) status = stop;
+        const int stop = *(const volatile int*)ctl->host_stop;    // cancel / time limit from the host, for THIS solve
+        if ((stop >> 3) == ctl->gen && (stop & 7)) status = stop & 7;
         else if (k >= ctl->limit) status = UC_ITERATION_LIMIT;
         if (status >= 0 && !ctl->fixed) ret_avg = have_avg && rk_avg < rk_cur;    // best of cur / avg
     }

@@ -57,7 +57,11 @@ struct uc_lp {
     // host <-> device mailboxes (pinned, mapped)
     HostStatus* h_status = nullptr; HostStatus* d_status = nullptr;
     int* h_stop = nullptr; int* d_stop = nullptr;
+    // cancel protocol (uc_pdhg_cancel): `state` = (generation << 1) | busy, changed only by solve entry / exit.  A
+    // cancel that finds a solve in flight stamps the stop flag with THAT solve's generation (a later solve ignores
+    // it); a cancel that finds the handle idle is kept for the next solve (cancel_requested).
     std::atomic<int> cancel_requested{0};
+    std::atomic<unsigned> state{0};
     std::atomic<int> busy{0};
     // one-time scalars
     double eta0 = 1.0, omega0 = 1.0, norm_b = 0.0, norm_c = 0.0;
@@ -244,6 +248,7 @@ void start_run(uc_lp* lp, const uc_pdhg_params& prm, cudaStream_t st, long long 
     h.beta_a = prm.beta_artificial; h.smoothing = prm.weight_smoothing; h.norm_q = lp->norm_b; h.norm_c = lp->norm_c;
     h.att = d_att; h.att_cap = d_att ? prm.attempt_trace_cap : 0; h.chk = d_chk; h.chk_cap = d_chk ? prm.check_trace_cap : 0;
     h.host_stop = lp->d_stop; h.host_status = lp->d_status; h.powtab = lp->powtab;
+    h.gen = (int)((lp->state.load() >> 1) & 0x0fffffffu);
     CK(cudaMemcpyAsync(lp->ctl, &h, sizeof(Ctrl), cudaMemcpyHostToDevice, st));
     k_init_point<<<lp->V.gridR, kBlock, 0, st>>>(lp->V, dx0, dy0, lp->perm_c, lp->perm_r);
     launch_kkt(lp, st, kModeInit);
@@ -613,8 +618,9 @@ int uc_lp_update_bounds(uc_lp* lp, const double* l_new, const double* u_new) {
 
 int uc_pdhg_cancel(uc_lp* lp) {
     if (!lp) return fail(UC_ERR_INVALID, "handle is NULL");
-    lp->cancel_requested.store(1);
-    if (lp->h_stop) { *(volatile int*)lp->h_stop = UC_CANCELLED; }
+    const unsigned st = lp->state.load();
+    if ((st & 1u) && lp->h_stop) __atomic_store_n(lp->h_stop, (int)(((st >> 1) & 0x0fffffffu) << 3) | UC_CANCELLED, __ATOMIC_SEQ_CST);
+    else lp->cancel_requested.store(1);
     return UC_OK;
 }
 
@@ -631,6 +637,7 @@ static int solve_impl(uc_lp* lp, const uc_pdhg_params* pin, double* x_out, doubl
     std::memset(res, 0, sizeof *res);
     const double t_wall = now_s();
     int rc = UC_OK;
+    bool in_flight = false;
     double *tx0 = nullptr, *ty0 = nullptr, *tx = nullptr, *ty = nullptr;
     uc_attempt_record* d_att = nullptr; uc_check_record* d_chk = nullptr;
     try {
@@ -641,16 +648,19 @@ static int solve_impl(uc_lp* lp, const uc_pdhg_params* pin, double* x_out, doubl
         const long long limit = fixed ? prm.fixed_iterations : prm.iter_limit;
         const int ce = prm.check_every;
 
-        // a cancel that arrived before the solve started is honoured here (PAPER.md l.80-85 race)
+        // a cancel that arrived while the handle was idle is honoured here (PAPER.md l.80-85 race): nothing runs,
+        // x_out / y_out are left untouched
         if (lp->cancel_requested.exchange(0)) {
-            *(volatile int*)lp->h_stop = 0;
             res->status = UC_CANCELLED;
             res->solve_seconds = now_s() - t_wall;
             lp->busy.store(0);
             return UC_OK;
         }
-        *(volatile int*)lp->h_stop = 0;
-        if (lp->cancel_requested.load()) *(volatile int*)lp->h_stop = UC_CANCELLED;   // cancel raced with the reset
+        // from here on uc_pdhg_cancel stamps the stop flag with this solve's generation
+        const unsigned gen = ((lp->state.load() >> 1) + 1u) & 0x0fffffffu;
+        lp->state.store((gen << 1) | 1u);
+        in_flight = true;
+        const int my_cancel = (int)(gen << 3) | UC_CANCELLED, my_timeout = (int)(gen << 3) | UC_TIME_LIMIT;
         std::memset(lp->h_status, 0, sizeof(HostStatus));
 
         // warm start
@@ -686,7 +696,12 @@ static int solve_impl(uc_lp* lp, const uc_pdhg_params* pin, double* x_out, doubl
             if (b >= depth - 1) {
                 CK(cudaEventSynchronize(lp->ev[(b - depth + 1) % depth]));
                 if (((volatile HostStatus*)lp->h_status)->done) done = true;
-                if (!done && now_s() - t_wall > prm.time_limit_s && *(volatile int*)lp->h_stop == 0) *(volatile int*)lp->h_stop = UC_TIME_LIMIT;
+                // a cancel that saw the handle idle just as this solve started
+                if (!done && lp->cancel_requested.exchange(0)) __atomic_store_n(lp->h_stop, my_cancel, __ATOMIC_SEQ_CST);
+                if (!done && now_s() - t_wall > prm.time_limit_s) {      // never overwrites a cancel of this solve
+                    int cur = __atomic_load_n(lp->h_stop, __ATOMIC_SEQ_CST);
+                    if (cur != my_cancel) __atomic_compare_exchange_n(lp->h_stop, &cur, my_timeout, false, __ATOMIC_SEQ_CST, __ATOMIC_SEQ_CST);
+                }
             }
         }
         CK(cudaStreamSynchronize(st));
@@ -732,9 +747,6 @@ static int solve_impl(uc_lp* lp, const uc_pdhg_params* pin, double* x_out, doubl
         res->loop_seconds = ms * 1e-3;
         res->attempt_records = hc.k; res->check_records = hc.nchk;
         res->kernel_launches = launches;
-        if (hc.status == UC_CANCELLED) lp->cancel_requested.store(0);
-        *(volatile int*)lp->h_stop = 0;
-        if (lp->cancel_requested.load()) *(volatile int*)lp->h_stop = UC_CANCELLED;   // arrived after the last check: stays sticky
     } catch (const CudaFail& f) {
         rc = fail((f.e == cudaErrorMemoryAllocation) ? UC_ERR_NOMEM : UC_ERR_CUDA, std::string(f.what) + ": " + cudaGetErrorString(f.e));
     }
@@ -745,6 +757,12 @@ static int solve_impl(uc_lp* lp, const uc_pdhg_params* pin, double* x_out, doubl
     if (d_att) cudaFree(d_att);
     if (d_chk) cudaFree(d_chk);
     res->solve_seconds = now_s() - t_wall;
+    if (in_flight) {
+        // the solve is over: a cancel stamped with its generation is stale from now on (it cannot leak into the next
+        // solve), and one that slipped into cancel_requested while it was starting is consumed with it
+        lp->state.store(lp->state.load() & ~1u);
+        lp->cancel_requested.store(0);
+    }
     lp->busy.store(0);
     return rc;
 }
@@ -767,6 +785,7 @@ int uc_pdhg_time_kernels(uc_lp* lp, void* stream, int32_t attempts, double* prim
         cudaStream_t st = stream ? (cudaStream_t)stream : lp->own_stream;
         uc_pdhg_params prm; uc_pdhg_default_params(&prm);
         const int warm = 8;
+        ensure_powtab(lp, (long long)attempts + warm);      // start_run only sizes the table for the launch loop of a solve
         start_run(lp, prm, st, (long long)attempts + warm, true, nullptr, nullptr, nullptr, nullptr);
         for (int i = 0; i < warm; ++i) launch_attempt(lp, st);
         ev.resize((size_t)2 * attempts + 1);

@@ -1,7 +1,7 @@
 """Algorithm 1 of the paper: race the GPU PDHG solver against a CPU LP solver on the same
 relaxed problem and terminate the loser.
 
-    1  partition the CPU cores between the two pipelines                     (l.70; here: `cpu_threads`)
+    1  partition the CPU cores between the two pipelines                     (l.70; here: `cpu_cores`, `gpu_host_cores`)
     2  start pipeline 1: PDHG on the GPU                                      (l.74)
     3  start pipeline 2: the CPU competitor                                   (l.77)
     4  while neither has converged: sleep `poll_s` (0.5 s in the paper, l.81)
@@ -16,6 +16,7 @@ out of scope.
 from __future__ import annotations
 
 import multiprocessing as mp
+import os
 import threading
 import time
 from dataclasses import dataclass, field
@@ -38,8 +39,30 @@ class RaceResult:
     log: list = field(default_factory=list)
 
 
-def _child(fn, args, q):
+def partition_cores(total: Optional[int] = None):
+    """Line 1 of Algorithm 1 ("Partition 48 CPU cores evenly between two solver instances"): the cores
+    this process may run on, split evenly -- (cores of the GPU pipeline's host thread, cores of the CPU competitor).
+    With fewer than two cores both sides get everything."""
     try:
+        avail = sorted(os.sched_getaffinity(0))
+    except AttributeError:                      # not Linux
+        avail = list(range(os.cpu_count() or 1))
+    if total is not None:
+        avail = avail[:max(1, int(total))]
+    if len(avail) < 2:
+        return set(avail), set(avail)
+    half = len(avail) // 2
+    return set(avail[:half]), set(avail[half:])
+
+
+def _child(fn, args, q, cores):
+    try:
+        if cores:
+            try:
+                os.sched_setaffinity(0, cores)          # the competitor's threads inherit it
+                os.environ["OMP_NUM_THREADS"] = str(len(cores))
+            except (AttributeError, OSError):
+                pass
         q.put(("ok", fn(*args)))
     except BaseException as e:      # the parent must never wait for a dead child
         q.put(("error", repr(e)))
@@ -47,33 +70,59 @@ def _child(fn, args, q):
 
 def race(handle: "_b.UcLp", competitor: Callable[..., Any], competitor_args: tuple = (), *,
          competitor_objective: Callable[[Any], float] = lambda r: float(r),
-         poll_s: float = 0.5, solve_kwargs: Optional[dict] = None, mp_context: str = "fork") -> RaceResult:
+         poll_s: float = 0.5, solve_kwargs: Optional[dict] = None, mp_context: str = "fork",
+         cpu_cores: Optional[set] = None, gpu_host_cores: Optional[set] = None) -> RaceResult:
     """Run Algorithm 1.  `handle` is a created UcLp (the LP is already on the GPU: presolve and model building
     are upstream of this library); `competitor(*competitor_args)` solves the same LP on the host and returns
-    something `competitor_objective` can turn into the optimal objective value."""
+    something `competitor_objective` can turn into the optimal objective value.
+    `cpu_cores` / `gpu_host_cores` (line 1, P:l.70): CPU sets the competitor process and the thread that drives
+    uc_pdhg_solve are pinned to (os.sched_setaffinity); None = no pinning; `partition_cores()` gives the paper's
+    even split.  The loop ends when the GPU side returns OPTIMAL, when the competitor returns a solution, or when
+    both have finished; a GPU return with any other status (iteration limit, time limit, numerical error) is logged
+    and the competitor is waited for ("while neither has converged", P:l.80)."""
     solve_kwargs = dict(solve_kwargs or {})
     t0 = time.perf_counter()
     box: dict = {}
 
     def gpu_side():
-        box["sol"] = handle.solve(**solve_kwargs)
+        if gpu_host_cores:
+            try:
+                os.sched_setaffinity(threading.get_native_id(), gpu_host_cores)
+            except (AttributeError, OSError):
+                pass
+        try:
+            box["sol"] = handle.solve(**solve_kwargs)
+        except BaseException as e:      # the poll loop must never wait for a dead thread
+            box["error"] = repr(e)
         box["t"] = time.perf_counter() - t0
 
     ctx = mp.get_context(mp_context)
     q = ctx.Queue()
-    proc = ctx.Process(target=_child, args=(competitor, competitor_args, q), daemon=True)
+    proc = ctx.Process(target=_child, args=(competitor, competitor_args, q, cpu_cores), daemon=True)
     th = threading.Thread(target=gpu_side, daemon=True)
     th.start()                       # line 2: pipeline 1
     proc.start()                     # line 3: pipeline 2
     res = RaceResult(winner="", objective=float("nan"), seconds=0.0)
     cpu_msg = None
-    while True:                      # line 4
+    gpu_logged = False
+    while True:                      # line 4: while neither has converged
         gpu_done = not th.is_alive()
         if cpu_msg is None and not q.empty():
             cpu_msg = q.get()
             res.cpu_seconds = time.perf_counter() - t0
-        if gpu_done or (cpu_msg is not None and cpu_msg[0] == "ok"):
+        gpu_conv = gpu_done and box.get("sol") is not None and box["sol"].status == _b.OPTIMAL
+        cpu_conv = cpu_msg is not None and cpu_msg[0] == "ok"
+        cpu_done = cpu_msg is not None or not proc.is_alive()
+        if gpu_conv or cpu_conv or (gpu_done and cpu_done):
+            if cpu_msg is None and not q.empty():                   # the child put its message just before exiting
+                cpu_msg = q.get()
+                res.cpu_seconds = time.perf_counter() - t0
             break
+        if gpu_done and not gpu_logged:                             # keep waiting for the competitor
+            gpu_logged = True
+            st = box["sol"].status if box.get("sol") is not None else None
+            res.log.append("gpu side returned without converging: " +
+                           (_b.STATUS_NAMES.get(st, str(st)) if st is not None else box.get("error", "no result")))
         if cpu_msg is not None and cpu_msg[0] == "error" and "competitor failed" not in " ".join(res.log):
             res.log.append("competitor failed: " + cpu_msg[1])     # keep waiting for the GPU side
         time.sleep(poll_s)
@@ -101,8 +150,10 @@ def race(handle: "_b.UcLp", competitor: Callable[..., Any], competitor_args: tup
             res.log.append("uc_pdhg_cancel sent")
     else:
         th.join()
-        proc.join(timeout=1.0)
-        raise RuntimeError(f"neither solver converged: gpu {box.get('sol')}, cpu {cpu_msg}")
+        if proc.is_alive():
+            proc.terminate()
+        proc.join(timeout=5.0)
+        raise RuntimeError(f"neither solver converged: gpu {box.get('sol') or box.get('error')}, cpu {cpu_msg}")
     proc.join(timeout=5.0)
     if th.is_alive():
         th.join()

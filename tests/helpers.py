@@ -101,3 +101,71 @@ def dense_kkt(lp, x, y):
 
 def rel_l2(a, b):
     return float(np.linalg.norm(np.asarray(a) - np.asarray(b)) / max(np.linalg.norm(b), 1e-300))
+
+
+def restart_replay(lp, sol, vs, beta_s=0.2, beta_n=0.8, beta_a=0.36, theta=0.5):
+    """Independent numpy restatement of DESIGN.md R9..R11 (restart decision and primal weight), fed ONLY with
+    iterates: `sol` is an oracle Solution with dump_checks (scaled current iterate, scaled average and w at every
+    check), `vs` the scaled matrix values K~ (pinned separately by the preconditioner tests).  Everything else is
+    recomputed here with dense algebra: the scaled data, omega0, KKT_omega of current / average / restart point,
+    candidate, restart kind, and the primal weight in its closed form
+        omega_new = (Dy / Dx)^theta * omega_old^(1 - theta)     (= sqrt(omega_old * Dy / Dx), the geometric mean, for
+                                                                 the default theta = 1/2).
+    Returns a list of dicts, one per check."""
+    m, n = lp.m, lp.n
+    Kt = np.zeros((m, n))
+    rows = np.repeat(np.arange(m), np.diff(lp.row_ptr))
+    Kt[rows, lp.col_idx] = vs
+    Dr, Dc = sol.Dr, sol.Dc
+    with np.errstate(invalid="ignore"):
+        c, q = lp.c / Dc, lp.b / Dr
+        l = np.where(lp.l <= -1e20, -np.inf, lp.l * Dc)
+        u = np.where(lp.u >= 1e20, np.inf, lp.u * Dc)
+    isE = lp.sense == ord("E")
+
+    def kkt_omega(x, y, omega):
+        a = Kt @ x - q
+        rp = np.where(isE, a, np.minimum(a, 0.0))
+        rho = c - Kt.T @ y
+        lam = np.maximum(rho, 0.0) * np.isfinite(l) + np.minimum(rho, 0.0) * np.isfinite(u)
+        rd = rho - lam
+        lo = np.where(np.isfinite(l), l, 0.0); hi = np.where(np.isfinite(u), u, 0.0)
+        dobj = q @ y + lo @ np.maximum(lam, 0.0) + hi @ np.minimum(lam, 0.0)
+        gap = c @ x - dobj
+        return float(np.sqrt(omega ** 2 * (rp @ rp) + (rd @ rd) / omega ** 2 + gap ** 2))
+
+    nc, nq = np.linalg.norm(c), np.linalg.norm(q)
+    omega = nc / nq if (nc > 1e-10 and nq > 1e-10) else 1.0
+    xr, yr = np.clip(np.zeros(n), l, u), np.zeros(m)
+    t0, mu_prev = 0, np.inf
+    out = []
+    for i, rec in enumerate(sol.checks[:len(sol.check_w)]):
+        k = int(rec["k"])
+        xc, yc, xa, ya, w = sol.check_x[i], sol.check_y[i], sol.check_avg_x[i], sol.check_avg_y[i], sol.check_w[i]
+        k_cur = kkt_omega(xc, yc, omega)
+        k_avg = kkt_omega(xa, ya, omega) if w > 0 else np.inf
+        cand = int(w > 0 and k_avg < k_cur)
+        zc = (xa, ya) if cand else (xc, yc)
+        mu_c, mu_r = (k_avg if cand else k_cur), kkt_omega(xr, yr, omega)
+        t = k - t0
+        kind = 0
+        if mu_c <= beta_s * mu_r:
+            kind = 1
+        elif mu_c <= beta_n * mu_r and mu_c > mu_prev:
+            kind = 2
+        elif t >= beta_a * k:
+            kind = 3
+        d = dict(k=k, kkt_cur=k_cur, kkt_avg=k_avg, candidate=cand, mu_c=mu_c, mu_r=mu_r, mu_prev=mu_prev, t=t,
+                 kind=kind, omega_before=omega, Dx=None, Dy=None)
+        if kind:
+            Dx, Dy = float(np.linalg.norm(zc[0] - xr)), float(np.linalg.norm(zc[1] - yr))
+            if Dx > 1e-10 and Dy > 1e-10:
+                omega = float(np.sqrt(omega * Dy / Dx)) if theta == 0.5 else float((Dy / Dx) ** theta * omega ** (1.0 - theta))
+            xr, yr = zc[0].copy(), zc[1].copy()
+            t0, mu_prev = k, np.inf
+            d.update(Dx=Dx, Dy=Dy)
+        else:
+            mu_prev = mu_c
+        d["omega_after"] = omega
+        out.append(d)
+    return out

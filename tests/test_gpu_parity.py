@@ -191,7 +191,12 @@ def test_convergence_parity_against_stored_oracle_runs(i):
     assert sg.status == P.OPTIMAL == gold["status"] and sg.rel_kkt <= 1e-4
     assert abs(sg.primal_obj - gold["primal_obj"]) <= TOL_OBJ * abs(gold["primal_obj"])
     assert abs(sg.dual_obj - gold["dual_obj"]) <= TOL_OBJ * abs(gold["dual_obj"])
-    assert abs(sg.iterations - gold["iterations"]) <= 0.1 * gold["iterations"]
+    # same terminating attempt, same restarts at the same checks with the same candidates
+    assert sg.iterations == gold["iterations"] and sg.accepted == gold["accepted"] and sg.restarts == gold["restarts"]
+    assert sg.returned_average == gold["returned_average"]
+    trace = [[int(c["k"]), int(c["restart_kind"]), int(c["candidate"])] for c in sg.checks if c["restart_kind"]]
+    assert trace == gold["restart_trace"]
+    assert sg.omega == pytest.approx(gold["omega"], rel=1e-9) and sg.eta == pytest.approx(gold["eta"], rel=1e-9)
     k = oracle.kkt_unscaled(lp, sg.x, sg.y)
     assert k["rel_kkt"] <= 1.0001e-4 and k["pobj"] == pytest.approx(sg.primal_obj, rel=1e-9)
 
@@ -216,6 +221,51 @@ def test_paper_scale_config3_trajectory_parity():
 def test_roofline_sweep_parity(seed, F):
     from workloads import sweep_config
     assert_trajectory_parity(sweep_config(seed), F)
+
+
+@pytest.mark.parametrize("seed", [12, 13, 14])
+def test_roofline_sweep_parity_200_attempts_against_stored_oracle(seed):
+    """BASELINE.json configs[4] at the 200 fixed attempts north_star states, m = n = 4e6 / 1e7 / 2e7 (checks and restarts
+    at k = 64, 128, 192 run at full size).  The oracle needs 3 / 11 / 25 minutes there, so its run is stored by
+    tests/golden/make_sweep_golden.py (oracle/ + workloads/ only): the full per-attempt trace -- every record holds
+    three reductions over ALL entries of the iterate --, the check trace, norms, seeded sample positions and seeded
+    random projections of x and y."""
+    from workloads import sweep_config
+    path = os.path.join(GOLDEN, f"oracle_sweep_seed{seed}.json")
+    gold = json.load(open(path))
+    lp = sweep_config(seed)
+    assert (lp.m, lp.n, lp.nnz) == (gold["m"], gold["n"], gold["nnz"])
+    F = gold["fixed_iterations"]
+    assert F == 200
+    with P.UcLp(lp) as h:
+        sg = h.solve(fixed_iterations=F, trace_attempts=F, trace_checks=64)
+    assert sg.iterations == F == gold["iterations"] and sg.accepted == gold["accepted"] and sg.restarts == gold["restarts"]
+    ga = gold["attempts"]
+    np.testing.assert_array_equal(sg.attempts["accepted"], np.array(ga["accepted"]))
+    for key in ("eta_used", "eta_next", "dx2", "dy2", "inter"):
+        np.testing.assert_allclose(sg.attempts[key], np.array(ga[key]), rtol=1e-9, atol=0, err_msg=key)
+    assert len(sg.checks) == len(gold["checks"]) == 3
+    for c, g in zip(sg.checks, gold["checks"]):
+        assert (int(c["k"]), int(c["restart_kind"]), int(c["candidate"])) == (g["k"], g["restart_kind"], g["candidate"])
+        assert c["omega_after"] == pytest.approx(g["omega_after"], rel=1e-9)
+        assert c["mu_c"] == pytest.approx(g["mu_c"], rel=1e-8) and c["mu_r"] == pytest.approx(g["mu_r"], rel=1e-8)
+    # sampled outputs: relative L2 over the sample, against the norm of the oracle's sample
+    ix, iy = np.array(gold["x_pos"]), np.array(gold["y_pos"])
+    assert rel_l2(sg.x[ix], np.array(gold["x_val"])) <= TOL_ITER
+    assert rel_l2(sg.y[iy], np.array(gold["y_val"])) <= TOL_ITER
+    assert np.linalg.norm(sg.x) == pytest.approx(gold["x_norm"], rel=1e-10)
+    assert np.linalg.norm(sg.y) == pytest.approx(gold["y_norm"], rel=1e-10)
+    # random projections r.x, s.y with r, s ~ N(0,1): |r.(x - x_o)| <= ~|x - x_o|, so 1e-10 |x| bounds the difference
+    for q in range(len(gold["x_proj"])):
+        for v, which, ref, nrm in ((sg.x, 0, gold["x_proj"][q], gold["x_norm"]), (sg.y, 1, gold["y_proj"][q], gold["y_norm"])):
+            rng = np.random.default_rng(777 + 10 * q + which)
+            acc = 0.0
+            for s_ in range(0, v.size, 1 << 22):
+                r = rng.standard_normal(min(1 << 22, v.size - s_))
+                acc += float(np.sum((r * v[s_:s_ + r.size]).astype(np.longdouble)))
+            assert abs(acc - ref) <= 5e-10 * nrm, (q, which)
+    assert sg.eta == pytest.approx(gold["eta"], rel=1e-9) and sg.omega == pytest.approx(gold["omega"], rel=1e-9)
+    assert sg.primal_obj == pytest.approx(gold["primal_obj"], rel=1e-9)
 
 
 def _host_gb():

@@ -11,7 +11,7 @@ import oracle
 from workloads import tiny, uc_config, fix_commitment
 from workloads.lp import from_dense
 
-from helpers import read_golden_rows, vertex_enumeration, highs, dense_kkt, rel_l2
+from helpers import read_golden_rows, vertex_enumeration, highs, dense_kkt, rel_l2, restart_replay
 
 
 def _f(s):
@@ -274,7 +274,141 @@ def test_average_is_eta_weighted_mean_of_accepted_iterates():
     assert s1.accepted == 3 and s1.iterations == 4
 
 
-# ------------------------------------------------------------------ R10/R11 invariants (decisions unpinned)
+# ------------------------------------------------------------------ R9..R11: restart rule and primal weight
+@pytest.mark.parametrize("name,l,u", [("free", -np.inf, np.inf), ("bounded", 0.0, 10.0)])
+def test_worked_restart_example_matches_golden(name, l, u):
+    """tests/golden/restart_1x1.txt (derivation: DESIGN.md 'Worked restart example'): 13 attempts with a check after
+    every one on two 1x1 LPs -- artificial, necessary and sufficient restarts, restarts to the average, a rejected
+    attempt between checks, and a primal weight that moves at every restart."""
+    rows = [r[1:] for r in read_golden_rows("restart_1x1.txt") if r[0] == name]
+    A = [r[1:] for r in rows if r[0] == "A"]
+    Cc = [r[1:] for r in rows if r[0] == "C"]
+    N = len(A)
+    assert N == len(Cc) == 13
+    # one attempt more than the golden holds: the check at the very last attempt of a run takes no restart decision
+    s = oracle.solve(tiny.one_by_one(l, u), fixed_iterations=N + 1, check_every=1, ruiz_iters=0, pc_alpha=0.0,
+                     trace_attempts=N, trace_checks=N, dump=N, dump_checks=N)
+    assert len(s.attempts) == N and len(s.checks) == N
+    R = dict(rel=2e-9, abs=1e-12)
+    x_start, y_start = 0.0, 0.0                       # the iterate attempt k starts from (R2 for k = 1)
+    kinds = set()
+    for i in range(N):
+        k, xt, yt, eta, ebar, acc, enext = int(A[i][0]), *map(_f, A[i][1:5]), int(A[i][5]), _f(A[i][6])
+        a = s.attempts[i]
+        assert k == i + 1 and a["accepted"] == acc, f"attempt {k}"
+        assert a["eta_used"] == pytest.approx(eta, **R) and a["eta_next"] == pytest.approx(enext, **R)
+        assert a["eta_bar"] == pytest.approx(ebar, **R) if math.isfinite(ebar) else math.isinf(a["eta_bar"])
+        # the iterate after attempt k (before the check): the trial point if accepted, else unchanged
+        exp_x, exp_y = (xt, yt) if acc else (x_start, y_start)
+        assert s.dump_x[i, 0] == pytest.approx(exp_x, **R) and s.dump_y[i, 0] == pytest.approx(exp_y, **R), f"attempt {k}"
+        assert s.check_x[i, 0] == pytest.approx(exp_x, **R) and s.check_y[i, 0] == pytest.approx(exp_y, **R)
+        kc, ka, cand, mu_c, mu_r, t, kind, om, xa, ya = (_f(Cc[i][1]), _f(Cc[i][2]), int(Cc[i][3]), _f(Cc[i][4]),
+                                                         _f(Cc[i][5]), int(Cc[i][6]), int(Cc[i][7]), _f(Cc[i][8]),
+                                                         _f(Cc[i][9]), _f(Cc[i][10]))
+        c = s.checks[i]
+        assert int(c["k"]) == k and c["restart_kind"] == kind, f"check {k}: kind {c['restart_kind']} != {kind}"
+        if kc != ka:                                   # printed values equal = a tie decided by the last bit
+            assert c["candidate"] == cand, f"check {k}"
+        assert c["mu_c"] == pytest.approx(mu_c, **R) and c["mu_r"] == pytest.approx(mu_r, **R), f"check {k}"
+        assert c["omega_after"] == pytest.approx(om, **R), f"check {k}"
+        # where the next attempt starts: the candidate on a restart (the average if it won), else the current iterate
+        if kind and c["candidate"]:
+            assert s.check_avg_x[i, 0] == pytest.approx(xa, **R) and s.check_avg_y[i, 0] == pytest.approx(ya, **R)
+        else:
+            assert exp_x == pytest.approx(xa, **R) and exp_y == pytest.approx(ya, **R)
+        x_start, y_start = xa, ya
+        kinds.add((kind, c["candidate"] if kind else -1))
+    assert {kd for kd, _ in kinds} == {0, 1, 2, 3}, "the example exercises no-restart and all three restart kinds"
+    assert (2, 1) in kinds                             # a restart TO THE AVERAGE is part of both examples
+
+
+def test_worked_restart_example_first_check_by_hand():
+    """Check 1 of the 'free' example re-derived here with plain floats (DESIGN.md carries it out in words):
+    z1 = (-1, 3): r_p = min(-1 - 1, 0) = -2, rho = 1 - 3 = -2 with no finite bound -> r_d = -2, pobj = -1, dobj = 3,
+    KKT_1 = sqrt(4 + 4 + 16); z_r = z0 = (0, 0): r_p = -1, r_d = 1, gap 0 -> sqrt(2); t = 1 >= 0.36 -> artificial;
+    Dx = 1, Dy = 3 -> omega = sqrt(1 * 3 / 1)."""
+    s = oracle.solve(tiny.one_by_one(-np.inf, np.inf), fixed_iterations=3, check_every=1, ruiz_iters=0, pc_alpha=0.0,
+                     trace_attempts=2, trace_checks=2)
+    c1, c2 = s.checks[:2]
+    assert c1["mu_c"] == pytest.approx(math.sqrt(24.0), rel=1e-15) and c1["mu_r"] == pytest.approx(math.sqrt(2.0), rel=1e-15)
+    assert c1["restart_kind"] == 3 and c1["candidate"] == 0
+    assert c1["omega_after"] == pytest.approx(math.sqrt(3.0), rel=1e-15)
+    # check 2 evaluates the NEW restart point (-1, 3) with the NEW omega = sqrt(3): sqrt(3 * 4 + 4 / 3 + 16)
+    assert c2["mu_r"] == pytest.approx(math.sqrt(12.0 + 4.0 / 3.0 + 16.0), rel=1e-15)
+
+
+REPLAY_CASES = {      # name -> (LP, attempts, check_every[, weight_smoothing])
+    "small_random_ce8": (lambda: tiny.small_random(6, 4, 1), 640, 8),
+    "small_random_theta02": (lambda: tiny.small_random(6, 4, 1), 640, 8, 0.2),
+    # the next two separate "mu_prev <- +inf on a restart" from a mu_prev that survives it (checks 4 / 4 would be kind 2)
+    "small_random_c_ce8": (lambda: tiny.small_random(7, 3, 0), 400, 8),
+    "small_random_ce3": (lambda: tiny.small_random(6, 4, 1), 399, 3),
+    "uc0_ce16_theta08": (lambda: uc_config(0), 800, 16, 0.8),
+    "small_random_b_ce5": (lambda: tiny.small_random(7, 3, 4), 640, 5),
+    "free_var_ce4": (tiny.free_var_lp, 400, 4),
+    "uc0": (lambda: uc_config(0), 640, 64),
+    "uc0_ce16": (lambda: uc_config(0), 1600, 16),
+}
+
+
+def _replay_case(case):
+    """R10 / R11 recomputed by helpers.restart_replay (dense numpy, closed-form geometric mean) from nothing but the
+    iterates the oracle dumped at each check: candidate, restart kind, mu_c, mu_r and omega of EVERY check must be the
+    oracle's.  A swapped Dy/Dx, theta vs 1 - theta, < vs <=, a stale omega in mu_r, a mu_prev that survives a restart
+    or a t that does not restart at t0 each change at least one of them."""
+    make, F, ce = REPLAY_CASES[case][:3]
+    theta = REPLAY_CASES[case][3] if len(REPLAY_CASES[case]) > 3 else 0.5
+    lp = make()
+    s = oracle.solve(lp, fixed_iterations=F + 1, check_every=ce, trace_attempts=F, trace_checks=F // ce, dump_checks=F // ce,
+                     weight_smoothing=theta)
+    assert len(s.checks) == F // ce == len(s.check_w)
+    vs, _, _ = oracle.precondition(lp)
+    rep = restart_replay(lp, s, vs, theta=theta)
+    seen = set()
+    n_cmp = 0
+    for r, c in zip(rep, s.checks):
+        k = r["k"]
+        if min(r["kkt_cur"], r["mu_r"]) < 1e-9:        # converged to round-off: the compared numbers are noise from here on
+            break
+        n_cmp += 1
+        tie_c = abs(r["kkt_avg"] - r["kkt_cur"]) <= 1e-11 * r["kkt_cur"] if np.isfinite(r["kkt_avg"]) else False
+        near = any(abs(r["mu_c"] - b * r["mu_r"]) <= 1e-11 * r["mu_r"] for b in (0.2, 0.8)) or \
+            (np.isfinite(r["mu_prev"]) and abs(r["mu_c"] - r["mu_prev"]) <= 1e-11 * r["mu_c"])
+        if not tie_c:
+            assert c["candidate"] == r["candidate"], f"check at k={k}"
+            assert c["mu_c"] == pytest.approx(r["mu_c"], rel=1e-9, abs=1e-13), f"k={k}"
+        assert c["mu_r"] == pytest.approx(r["mu_r"], rel=1e-9, abs=1e-13), f"k={k}"
+        if not (tie_c or near):
+            assert c["restart_kind"] == r["kind"], f"check at k={k}: oracle {c['restart_kind']}, replay {r['kind']} ({r})"
+        assert c["omega_after"] == pytest.approx(r["omega_after"], rel=1e-11), f"k={k}: Dx {r['Dx']} Dy {r['Dy']}"
+        seen.add((int(c["restart_kind"]), int(c["candidate"])))
+    assert n_cmp >= 10 or n_cmp == len(rep)
+    # w at a check = sum of the step sizes of the attempts accepted since the last restart (R6 + 'sums <- 0' of R11)
+    acc = s.attempts["accepted"] == 1
+    t0 = 0
+    for i, c in enumerate(s.checks):
+        k = int(c["k"])
+        sel = acc[t0:k]
+        assert s.check_w[i] == pytest.approx(s.attempts["eta_used"][t0:k][sel].sum(), rel=1e-12), f"k={k}"
+        if c["restart_kind"]:
+            t0 = k
+    return seen
+
+
+@pytest.mark.parametrize("case", list(REPLAY_CASES))
+def test_restart_decisions_and_primal_weight_recomputed_from_iterates(case):
+    _replay_case(case)
+
+
+def test_restart_replay_cases_cover_every_branch():
+    seen = set()
+    for case in REPLAY_CASES:
+        seen |= _replay_case(case)
+    kinds = {k for k, _ in seen}
+    assert kinds == {0, 1, 2, 3}, seen
+    assert {c for k, c in seen if k} == {0, 1}, "restarts to the current iterate and to the average both occur"
+
+
 def test_restart_and_primal_weight_invariants():
     lp = uc_config(0)
     s = oracle.solve(lp, fixed_iterations=640)

@@ -15,12 +15,13 @@ from paper_2607_03627_b200.race import race
 class StandInHandle:
     """Behaves like UcLp for race(): solve() blocks for `seconds` unless cancel() arrives first."""
 
-    def __init__(self, seconds, objective=1.25):
+    def __init__(self, seconds, objective=1.25, final_status=B.OPTIMAL):
         self.seconds, self.objective, self._stop, self.cancelled = seconds, objective, threading.Event(), False
+        self.final_status = final_status
 
     def solve(self, **kw):
         stopped = self._stop.wait(self.seconds)
-        status = B.CANCELLED if stopped else B.OPTIMAL
+        status = B.CANCELLED if stopped else self.final_status
         return SimpleNamespace(status=status, primal_obj=self.objective, iterations=0)
 
     def cancel(self):
@@ -64,6 +65,50 @@ def test_competitor_failure_does_not_hang_the_race():
     h = StandInHandle(seconds=0.3, objective=2.0)
     r = race(h, broken, (), poll_s=0.05)
     assert r.winner == "gpu_pdhg" and r.objective == 2.0
+
+
+@pytest.mark.parametrize("status", [B.ITERATION_LIMIT, B.TIME_LIMIT, B.NUMERICAL_ERROR])
+def test_gpu_side_returning_early_without_converging_does_not_end_the_race(status):
+    """Algorithm 1, P:l.80 "while neither has converged": a GPU return at its iteration limit is not a convergence;
+    the competitor is waited for and wins."""
+    h = StandInHandle(seconds=0.1, final_status=status)
+    r = race(h, slow_competitor, (0.6, 4.5), poll_s=0.05)
+    assert r.winner == "cpu" and r.objective == 4.5 and r.gpu.status == status
+    assert not h.cancelled and r.cancel_latency_s is None            # nothing left to cancel
+    assert any("without converging" in m for m in r.log)
+
+
+def test_neither_converges_raises_and_leaves_no_child_behind():
+    import multiprocessing as mp
+
+    def broken():
+        raise ValueError("no licence")
+    h = StandInHandle(seconds=0.1, final_status=B.ITERATION_LIMIT)
+    before = len(mp.active_children())
+    with pytest.raises(RuntimeError, match="neither solver converged"):
+        race(h, broken, (), poll_s=0.05)
+    assert len(mp.active_children()) <= before
+
+
+def _report_affinity():
+    import os
+    return sorted(os.sched_getaffinity(0))
+
+
+def test_core_partition_pins_the_competitor_process():
+    """Algorithm 1 line 1 (P:l.70): the cores are split evenly; the competitor process runs on its half only."""
+    import os
+    from paper_2607_03627_b200.race import partition_cores
+    gpu_cores, cpu_cores = partition_cores()
+    avail = os.sched_getaffinity(0)
+    assert gpu_cores | cpu_cores == set(avail)
+    if len(avail) >= 2:
+        assert not (gpu_cores & cpu_cores) and abs(len(gpu_cores) - len(cpu_cores)) <= 1
+    h = StandInHandle(seconds=30.0)
+    r = race(h, _report_affinity, (), competitor_objective=lambda cores: float(len(cores)), poll_s=0.05,
+             cpu_cores=cpu_cores, gpu_host_cores=gpu_cores)
+    assert r.winner == "cpu" and r.cpu == sorted(cpu_cores)
+    assert os.sched_getaffinity(0) == avail                          # the caller's own affinity is untouched
 
 
 @pytest.mark.gpu

@@ -11,9 +11,10 @@ from .lp import LP, from_dense
 INF = np.inf
 
 
-def one_by_one() -> LP:
-    """min x s.t. x >= 1, 0 <= x <= 10  (SURVEY 8(c) worked PDHG-step example; x*=1, y*=1)."""
-    return from_dense([[1.0]], ["G"], [1.0], [1.0], [0.0], [10.0], name="one_by_one")
+def one_by_one(l: float = 0.0, u: float = 10.0) -> LP:
+    """min x s.t. x >= 1, l <= x <= u; default 0 <= x <= 10 (SURVEY 8(c) worked PDHG-step example; x*=1, y*=1).
+    (l, u) = (-inf, inf) is the free-variable case of the worked restart example (tests/golden/restart_1x1.txt)."""
+    return from_dense([[1.0]], ["G"], [1.0], [1.0], [l], [u], name="one_by_one")
 
 
 def two_var() -> LP:
