@@ -61,7 +61,9 @@ typedef struct {
     int32_t sell_window;        /* rows per length-sorting window of the sliced-ELL layout; 4096 */
     int32_t long_row_threshold; /* rows longer than this leave the sliced-ELL part (warp-per-row); 32 */
     int32_t keep_source_map;    /* 1: keep the slot -> CSR position maps on the host (uc_lp_get_scaled_values); 0 */
-    int32_t pad_;
+    int32_t index_compression;  /* 1 (default): slices whose column indices span < 2^16 store them as 16-bit offsets from
+                                   the slice's smallest index (SURVEY.md 8(f) NEXT-4, 2 bytes per entry less per matrix
+                                   copy; results are bit-identical); 0: 32-bit indices everywhere */
 } uc_lp_options;
 
 void uc_lp_default_options(uc_lp_options* opt);
@@ -176,6 +178,7 @@ typedef struct {
     double eta0, omega0;                 /* R2 */
     double norm_b, norm_c;               /* unscaled 2-norms used by R9 */
     int64_t bytes_per_attempt;           /* bytes one attempt streams in this layout */
+    int64_t k_narrow_slots, kt_narrow_slots; /* stored slots whose column index is a 16-bit offset (index_compression) */
 } uc_lp_info;
 
 int uc_lp_get_info(const uc_lp* lp, uc_lp_info* info);

@@ -22,7 +22,7 @@ class UcError(RuntimeError):
 class Options(C.Structure):
     _fields_ = [("device", C.c_int32), ("ruiz_iters", C.c_int32), ("pc_alpha", C.c_double),
                 ("sell_window", C.c_int32), ("long_row_threshold", C.c_int32),
-                ("keep_source_map", C.c_int32), ("pad_", C.c_int32)]
+                ("keep_source_map", C.c_int32), ("index_compression", C.c_int32)]
 
 
 class Params(C.Structure):
@@ -51,7 +51,7 @@ class Info(C.Structure):
                 ("k_long_nnz", C.c_int64), ("kt_long_nnz", C.c_int64), ("device_bytes", C.c_int64),
                 ("precondition_seconds", C.c_double), ("create_seconds", C.c_double),
                 ("eta0", C.c_double), ("omega0", C.c_double), ("norm_b", C.c_double), ("norm_c", C.c_double),
-                ("bytes_per_attempt", C.c_int64)]
+                ("bytes_per_attempt", C.c_int64), ("k_narrow_slots", C.c_int64), ("kt_narrow_slots", C.c_int64)]
 
 
 ATTEMPT_DTYPE = np.dtype([("eta_used", "f8"), ("eta_bar", "f8"), ("eta_next", "f8"), ("dx2", "f8"),

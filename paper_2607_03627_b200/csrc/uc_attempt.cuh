@@ -43,8 +43,11 @@
 namespace ucpdhg {
 
 // build-time tunables (-DUC_...): the defaults are the measured optimum on config 3 (profiles/)
-#ifndef UC_ATT_WARPS
-#define UC_ATT_WARPS 15
+#ifndef UC_PRIMAL_WARPS
+#define UC_PRIMAL_WARPS 15     // consumer warps per CTA of k_primal
+#endif
+#ifndef UC_DUAL_WARPS
+#define UC_DUAL_WARPS 15       // consumer warps per CTA of k_dual
 #endif
 #ifndef UC_CTAS_PER_SM
 #define UC_CTAS_PER_SM 1
@@ -52,13 +55,17 @@ namespace ucpdhg {
 #ifndef UC_DB
 #define UC_DB 1
 #endif
-constexpr int kAttWarps = UC_ATT_WARPS;        // consumer warps per CTA
+constexpr int kPrimalWarps = UC_PRIMAL_WARPS, kDualWarps = UC_DUAL_WARPS;      // consumer warps per CTA
 constexpr int kCtasPerSm = UC_CTAS_PER_SM;
-constexpr int kAttemptThreads = (kAttWarps + 1) * 32;   // + long-row warp
-constexpr int kDB = UC_DB;                     // data (values, vectors, gathers) run kDB steps ahead of the compute
-constexpr int kDA = 2 * kDB + 1;               // indices run kDA steps ahead: a group is complete kDB commits later
-constexpr int kRingA = kDA - kDB + 1;          // slots of the index ring
-constexpr int kRingB = kDB + 1;                // slots of the data ring
+constexpr int kPrimalThreads = (kPrimalWarps + 1) * 32, kDualThreads = (kDualWarps + 1) * 32;   // + long-row warp
+// pipeline depth, per kernel: data (values, vectors, gathers) run kDB steps ahead of the compute, indices
+// kDA = 2 kDB + 1 steps ahead (a group is complete kDB commits later); kDB + 2 index slots, kDB + 1 data slots
+#ifndef UC_PRIMAL_DB
+#define UC_PRIMAL_DB UC_DB
+#endif
+#ifndef UC_DUAL_DB
+#define UC_DUAL_DB UC_DB
+#endif
 constexpr int kChunkE = kChunkT * 32;          // stored entries per step
 
 // ------------------------------------------------------------------------------------------ PTX
@@ -102,19 +109,21 @@ struct DataSlot {
     double vec[NVEC][32];        // 32-row segments of the per-row vectors (last step of a slice only)
     unsigned char bvec[BYTEVEC ? 32 : 16];
 };
-template <int NVEC, bool BYTEVEC, class GT>
+template <int NVEC, bool BYTEVEC, class GT, int DB>
 struct WarpRing {
+    static constexpr int kDB = DB, kDA = 2 * DB + 1, kRingA = DB + 2, kRingB = DB + 1;
     int col[kRingA][kChunkE];
     DataSlot<NVEC, BYTEVEC, GT> data[kRingB];
 };
-template <int NVEC, bool BYTEVEC, class GT>
+template <int NVEC, bool BYTEVEC, class GT, int WARPS, int DB>
 struct SmemT {
-    WarpRing<NVEC, BYTEVEC, GT> w[kAttWarps];
+    WarpRing<NVEC, BYTEVEC, GT, DB> w[WARPS];
     dd red[2 * 32];
 };
-using PrimalSmem = SmemT<5, false, double>;   // x, c, l, u, xsum ; gathers y
-using DualSmem = SmemT<3, true, double2>;     // y, q, ysum + isG ; gathers {xbar, dx}
-static_assert(kCtasPerSm * (sizeof(PrimalSmem) + 1024) <= 228 * 1024 && kCtasPerSm * (sizeof(DualSmem) + 1024) <= 228 * 1024,
+using PrimalSmem = SmemT<5, false, double, kPrimalWarps, UC_PRIMAL_DB>;   // x, c, l, u, xsum ; gathers y
+using DualSmem = SmemT<3, true, double2, kDualWarps, UC_DUAL_DB>;         // y, q, ysum + isG ; gathers {xbar, dx}
+constexpr size_t kPrimalSmemBytes = sizeof(PrimalSmem), kDualSmemBytes = sizeof(DualSmem);
+static_assert(kCtasPerSm * (kPrimalSmemBytes + 1024) <= 228 * 1024 && kCtasPerSm * (kDualSmemBytes + 1024) <= 228 * 1024,
               "the CTAs of either attempt kernel must fit the shared memory of one SM");
 
 // Calls f(std::integral_constant<int, nt>) for nt = 1..kChunkT (nothing for nt = 0).  nt is warp-uniform, so
@@ -145,16 +154,17 @@ __device__ __forceinline__ void dispatch_nt(int nt, F f) {
 template <class Ring, class GT, class FD, class FV, class FC>
 __device__ __forceinline__ bool warp_pipeline(const Sell& A, Ring& R, int gw, int lane, const GT* const& gsrc,
                                               uint64_t pol_first, FD dep_ready, FV issue_vecs, FC compute) {
+    constexpr int kDB = Ring::kDB, kDA = Ring::kDA, kRingA = Ring::kRingA, kRingB = Ring::kRingB;
     int J = A.steps_per_warp;                                      // shrinks to this warp's own count at its end marker
     const long long GW = A.sched_warps;
-    auto load_desc = [&](int k) -> int2 {
-        return k < J ? __ldg(reinterpret_cast<const int2*>(A.steps + (long long)k * GW + gw)) : make_int2(0, 0);
+    auto load_desc = [&](int k) -> int4 {
+        return k < J ? __ldg(reinterpret_cast<const int4*>(A.steps + (long long)k * GW + gw)) : make_int4(0, 0, -1, 0);
     };
-    int2 dcur = load_desc(lane), dnxt = load_desc(32 + lane);
-    long long qa_e[kDA - kDB]; int qa_i[kDA - kDB], qa_r[kDA - kDB];     // A -> B
+    int4 dcur = load_desc(lane), dnxt = load_desc(32 + lane);
+    long long qa_e[kDA - kDB]; int qa_i[kDA - kDB], qa_r[kDA - kDB], qa_c[kDA - kDB];     // A -> B
     int qb_i[kDB], qb_r[kDB];                                            // B -> C
 #pragma unroll
-    for (int q = 0; q < kDA - kDB; ++q) { qa_e[q] = 0; qa_i[q] = 0; qa_r[q] = 0; }
+    for (int q = 0; q < kDA - kDB; ++q) { qa_e[q] = 0; qa_i[q] = 0; qa_r[q] = 0; qa_c[q] = -1; }
 #pragma unroll
     for (int q = 0; q < kDB; ++q) { qb_i[q] = 0; qb_r[q] = 0; }
     // ring slots of steps ka (index ring), kb (index ring: kb = ka - (kRingA - 1)), kb (data ring: kb = -kRingB at the start), j
@@ -167,14 +177,16 @@ __device__ __forceinline__ bool warp_pipeline(const Sell& A, Ring& R, int gw, in
         const int src_lane = ka & 31;
         const unsigned w0 = (unsigned)__shfl_sync(0xffffffffu, dcur.x, src_lane);
         const int row_a = __shfl_sync(0xffffffffu, dcur.y, src_lane), info_a = (int)(w0 >> 26);
+        const int cb_a = __shfl_sync(0xffffffffu, dcur.z, src_lane);       // >= 0: 16-bit offsets from cb_a (uc_format.hpp)
         const long long eb_a = (long long)(w0 & 0x3ffffffu) << 5;
         if (info_a & kStepEnd) J = min(J, ka);
-        if (lane < (info_a & 7) * 8) cp_stream16(&R.col[sa][lane * 4], A.col + eb_a + lane * 4, pol_first);
+        if (cb_a >= 0) { if (lane < (info_a & 7) * 4) cp_stream16(&R.col[sa][lane * 4], A.col16 + eb_a + lane * 8, pol_first); }
+        else if (lane < (info_a & 7) * 8) cp_stream16(&R.col[sa][lane * 4], A.col + eb_a + lane * 4, pol_first);
         // ---- B: values, vectors and gathers of step kb = j + kDB (its indices landed kDB commits ago)
-        const long long eb = qa_e[0]; const int info_b = qa_i[0], row_b = qa_r[0];
+        const long long eb = qa_e[0]; const int info_b = qa_i[0], row_b = qa_r[0], cb_b = qa_c[0];
 #pragma unroll
-        for (int q = 0; q + 1 < kDA - kDB; ++q) { qa_e[q] = qa_e[q + 1]; qa_i[q] = qa_i[q + 1]; qa_r[q] = qa_r[q + 1]; }
-        qa_e[kDA - kDB - 1] = eb_a; qa_i[kDA - kDB - 1] = info_a; qa_r[kDA - kDB - 1] = row_a;
+        for (int q = 0; q + 1 < kDA - kDB; ++q) { qa_e[q] = qa_e[q + 1]; qa_i[q] = qa_i[q + 1]; qa_r[q] = qa_r[q + 1]; qa_c[q] = qa_c[q + 1]; }
+        qa_e[kDA - kDB - 1] = eb_a; qa_i[kDA - kDB - 1] = info_a; qa_r[kDA - kDB - 1] = row_a; qa_c[kDA - kDB - 1] = cb_a;
         {
             const int nt = info_b & 7;
             auto& D = R.data[sb];
@@ -184,10 +196,11 @@ __device__ __forceinline__ bool warp_pipeline(const Sell& A, Ring& R, int gw, in
                 if (p < nt * 16) cp_stream16(&D.val[p * 2], A.val + eb + p * 2, pol_first);
             }
             if (info_b & kStepLast) issue_vecs(D, row_b);
+            const unsigned short* c16 = reinterpret_cast<const unsigned short*>(R.col[sbA]);
             dispatch_nt(nt, [&](auto n) {
                 int c[decltype(n)::value];
 #pragma unroll
-                for (int t = 0; t < decltype(n)::value; ++t) c[t] = R.col[sbA][t * 32 + lane];
+                for (int t = 0; t < decltype(n)::value; ++t) c[t] = cb_b >= 0 ? cb_b + (int)c16[t * 32 + lane] : R.col[sbA][t * 32 + lane];
 #pragma unroll
                 for (int t = 0; t < decltype(n)::value; ++t) cp_gather(&D.gv[t * 32 + lane], gsrc + c[t]);
             });
@@ -247,9 +260,10 @@ __device__ __forceinline__ double primal_update(const Vecs& V, double* __restric
     return dx * dx;
 }
 
-__global__ void __launch_bounds__(kAttemptThreads, kCtasPerSm) k_primal(Sell KT, Vecs V, Ctrl* ctl) {
+__global__ void __launch_bounds__(kPrimalThreads, kCtasPerSm) k_primal(Sell KT, Vecs V, Ctrl* ctl) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     PrimalSmem& P = *reinterpret_cast<PrimalSmem*>(smem_raw);
+    dd* const red = P.red;
     grid_launch_dependents();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     dd acc[1] = {dd{0.0, 0.0}};
@@ -274,7 +288,7 @@ __global__ void __launch_bounds__(kAttemptThreads, kCtasPerSm) k_primal(Sell KT,
         return true;
     };
 
-    if (warp == kAttWarps) {                               // ---- long rows, one per pass
+    if (warp == kPrimalWarps) {                               // ---- long rows, one per pass
         if (!dep_ready()) return;
         for (int r = blockIdx.x; r < KT.nlong; r += gridDim.x) {
             const long long j = KT.nshort + r;
@@ -286,7 +300,7 @@ __global__ void __launch_bounds__(kAttemptThreads, kCtasPerSm) k_primal(Sell KT,
         }
     } else {                                               // ---- consumer warps
         double g[1] = {0.0};
-        const bool live = warp_pipeline(KT, P.w[warp], (int)blockIdx.x * kAttWarps + warp, lane, ycur, pol.first, dep_ready,
+        const bool live = warp_pipeline(KT, P.w[warp], (int)blockIdx.x * kPrimalWarps + warp, lane, ycur, pol.first, dep_ready,
             [&](auto& D, int row0) {                       // x, c, l, u (, xsum): 16 pieces of 16 bytes each
 #pragma unroll
                 for (int k = 0; k < 3; ++k)
@@ -305,7 +319,7 @@ __global__ void __launch_bounds__(kAttemptThreads, kCtasPerSm) k_primal(Sell KT,
             });
         if (!live) return;
     }
-    block_sum_dd<1>(acc, P.red);
+    block_sum_dd<1>(acc, red);
     if (threadIdx.x == 0) V.partA[blockIdx.x] = acc[0];
 }
 
@@ -321,9 +335,10 @@ __device__ __forceinline__ double dual_update(const Vecs& V, double* __restrict_
     return yn - r.y;
 }
 
-__global__ void __launch_bounds__(kAttemptThreads, kCtasPerSm) k_dual(Sell K, Vecs V, Ctrl* ctl) {
+__global__ void __launch_bounds__(kDualThreads, kCtasPerSm) k_dual(Sell K, Vecs V, Ctrl* ctl) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     DualSmem& P = *reinterpret_cast<DualSmem*>(smem_raw);
+    dd* const red = P.red;
     grid_launch_dependents();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     dd acc[2] = {dd{0.0, 0.0}, dd{0.0, 0.0}};
@@ -333,17 +348,20 @@ __global__ void __launch_bounds__(kAttemptThreads, kCtasPerSm) k_dual(Sell K, Ve
     int cur = 0, pend = 0; double eta_prev = 0.0, sig = 0.0;
     const double* ycur = nullptr; double* ynext = nullptr;
     const double* vsrc[2]; int voff[2]; bool vok[2];   // this lane's share of a slice's vector segments
-    // inputs of the step rule (A9), fetched by thread 0 of every CTA while the kernel starts: whichever CTA finishes
-    // last then runs the rule without a single cold load on the critical path of the whole solve
-    double r_eta = 0.0, r_omega = 0.0, r_w = 0.0; long long r_k = 0, r_acc = 0, r_cap = 0;
-    double2 r_pw = make_double2(0.0, 0.0); uc_attempt_record* r_att = nullptr;
+    // inputs of the step rule (A9), fetched by thread 0 of every CTA while the kernel starts and parked in shared
+    // memory: whichever CTA finishes last then runs the rule without a single cold load on the critical path of the
+    // whole solve
+    struct RuleIn { double eta, omega, w; long long k, acc, cap; double2 pw; uc_attempt_record* att; };
+    __shared__ RuleIn rule_in;
     auto dep_ready = [&]() -> bool {
         grid_dependency_wait();
         if (ld_flag(&ctl->done)) return false;
         cur = ctl->cur; pend = ctl->pending; eta_prev = ctl->eta_prev; sig = ctl->eta * ctl->omega;
         if (threadIdx.x == 0) {
-            r_eta = ctl->eta; r_omega = ctl->omega; r_w = ctl->w; r_k = ctl->k; r_acc = ctl->accepted;
-            r_att = ctl->att; r_cap = ctl->att_cap; r_pw = ctl->powtab[r_k];     // {(k+1)^-0.6, (k+1)^-0.3} of attempt k = r_k + 1
+            RuleIn r;
+            r.eta = ctl->eta; r.omega = ctl->omega; r.w = ctl->w; r.k = ctl->k; r.acc = ctl->accepted;
+            r.att = ctl->att; r.cap = ctl->att_cap; r.pw = ctl->powtab[r.k];     // {(k+1)^-0.6, (k+1)^-0.3} of attempt k = r.k + 1
+            rule_in = r;
         }
         ycur = V.y[cur]; ynext = V.y[cur ^ 1];
 #pragma unroll
@@ -355,7 +373,7 @@ __global__ void __launch_bounds__(kAttemptThreads, kCtasPerSm) k_dual(Sell K, Ve
         return true;
     };
 
-    if (warp == kAttWarps) {                               // ---- long rows
+    if (warp == kDualWarps) {                               // ---- long rows
         if (!dep_ready()) return;
         auto gather = [&](int c, double (&o)[2]) { const double2 t = __ldg(xg + c); o[0] = t.x; o[1] = t.y; };
         for (int r = blockIdx.x; r < K.nlong; r += gridDim.x) {
@@ -371,7 +389,7 @@ __global__ void __launch_bounds__(kAttemptThreads, kCtasPerSm) k_dual(Sell K, Ve
         }
     } else {                                               // ---- consumer warps
         double kx[2] = {0.0, 0.0};
-        const bool live = warp_pipeline(K, P.w[warp], (int)blockIdx.x * kAttWarps + warp, lane, xg, pol.first, dep_ready,
+        const bool live = warp_pipeline(K, P.w[warp], (int)blockIdx.x * kDualWarps + warp, lane, xg, pol.first, dep_ready,
             [&](auto& D, int row0) {                       // y, q (, ysum): 16 pieces each; isG: 2 pieces
 #pragma unroll
                 for (int k = 0; k < 2; ++k)
@@ -392,7 +410,7 @@ __global__ void __launch_bounds__(kAttemptThreads, kCtasPerSm) k_dual(Sell K, Ve
             });
         if (!live) return;
     }
-    block_sum_dd<2>(acc, P.red);
+    block_sum_dd<2>(acc, red);
     // ---- A9: the last CTA finishes the reductions and runs the step-size rule (R5).  This is the serial tail of
     // every attempt (measured: 8.6 us of 88 on config 3, 6.2 of 16 on config 1, before this form), so it is ONE warp,
     // shuffles only, no block barrier, no cold load: the other warps are gone as soon as the block sum is done.
@@ -429,6 +447,9 @@ __global__ void __launch_bounds__(kAttemptThreads, kCtasPerSm) k_dual(Sell K, Ve
     if (lane != 0) return;
     ctl->ticket_b = 0;
     const double dx2 = dd_round(s3[0]), dy2 = dd_round(s3[1]), inter = fabs(dd_round(s3[2]));
+    const double r_eta = rule_in.eta, r_omega = rule_in.omega, r_w = rule_in.w;      // written by this very thread
+    const long long r_k = rule_in.k, r_acc = rule_in.acc, r_cap = rule_in.cap;
+    const double2 r_pw = rule_in.pw; uc_attempt_record* const r_att = rule_in.att;
     const double eta = r_eta, omega = r_omega;
     const long long k = r_k + 1;
     const double N = omega * dx2 + dy2 / omega;

@@ -19,22 +19,25 @@
 #include <utility>
 #include <thread>
 #include <cmath>
+#include <climits>
 
 namespace ucpdhg {
 
 // One step of the warp-private pipelines of the persistent attempt kernels (uc_attempt.cuh): a chunk of at
 // most kChunkT entries per row of one slice.  A slice wider than kChunkT is a run of consecutive steps of
-// the same warp, the row sums carried in registers from one to the next.  8 bytes.
+// the same warp, the row sums carried in registers from one to the next.  16 bytes.
 constexpr int kChunkT = 4;
 struct StepDesc {
     uint32_t w0;       // bits 0-25: (first stored entry of the chunk in the sliced-ELL arrays) / 32; bits 26-31: info
     int32_t row0;      // first row of the slice
+    int32_t cbase;     // >= 0: the slice's column indices are stored as 16-bit offsets from cbase; -1: as 32-bit indices
+    int32_t pad_;
 };
 // info: bits 0-2 entries per row in this chunk (0 = padding step: nothing to do)
 constexpr int kStepFirst = 8;    // first chunk of its slice
 constexpr int kStepLast = 16;    // last chunk of its slice (the update is applied)
 constexpr int kStepEnd = 32;     // the warp has no further steps (set on its first padding step)
-static_assert(sizeof(StepDesc) == 8, "StepDesc layout");
+static_assert(sizeof(StepDesc) == 16, "StepDesc layout");
 
 // f(begin, end) over [0, n) on up to 8 host threads (uc_lp_create is a one-time cost, but it is inside the
 // end-to-end time: the layouts of a 6M-entry matrix take ~0.5 s on one core)
@@ -55,7 +58,11 @@ inline void parallel_ranges(int64_t n, int64_t grain, F f) {
 struct HostSell {
     int64_t nrows = 0, nshort = 0, nlong = 0, nslices = 0;
     std::vector<int64_t> slice_ptr;   // [nslices+1]
-    std::vector<int32_t> col;         // [slots]
+    std::vector<int32_t> col;         // [slots]  column indices (the reference; uploaded only if some slice is wide)
+    std::vector<uint16_t> col16;      // [slots]  16-bit offsets from cbase[slice] (uploaded only if some slice is narrow)
+    std::vector<int32_t> cbase;       // [nslices] smallest column index of a narrow slice, -1 for a wide one
+    int64_t narrow_slots = 0;         // stored slots (incl. padding) of the narrow slices
+    std::vector<int32_t> rlen;        // [nshort] entries of each row of the sliced part
     std::vector<double> val;          // [slots]
     std::vector<int64_t> src;         // [slots]  caller's CSR position of the slot, -1 = padding (only if asked for)
     std::vector<int64_t> lptr;        // [nlong+1]
@@ -96,7 +103,7 @@ inline void build_schedule(HostSell& S, int64_t warps) {
     int64_t J = 0;
     for (int64_t c : count) J = std::max(J, c);
     S.steps_per_warp = J;
-    S.steps.assign((size_t)(J * warps), StepDesc{0u, 0});
+    S.steps.assign((size_t)(J * warps), StepDesc{0u, 0, -1, 0});
     std::fill(count.begin(), count.end(), 0);
     for (int64_t s = 0; s < S.nslices; ++s) {
         const int64_t wd = (S.slice_ptr[(size_t)s + 1] - S.slice_ptr[(size_t)s]) / 32;
@@ -108,6 +115,7 @@ inline void build_schedule(HostSell& S, int64_t warps) {
             const uint32_t info = (uint32_t)std::max<int64_t>(nt, 0) | (c == 0 ? kStepFirst : 0) | (c == nch - 1 ? kStepLast : 0);
             d.w0 = (uint32_t)((S.slice_ptr[(size_t)s] + 32 * kChunkT * c) >> 5) | (info << 26);   // slots < 2^31 (checked at create)
             d.row0 = (int32_t)(32 * s);
+            d.cbase = S.cbase.empty() ? -1 : S.cbase[(size_t)s]; d.pad_ = 0;
             S.steps[(size_t)(count[(size_t)w]++ * warps + w)] = d;
         }
     }
@@ -166,9 +174,11 @@ inline void build_sell(int64_t nrows, const int64_t* ptr, const int32_t* idx, co
     const int64_t slots = S.slice_ptr[(size_t)S.nslices];
     S.col.assign((size_t)slots, 0); S.val.assign((size_t)slots, 0.0);
     if (want_src) S.src.assign((size_t)slots, -1);
+    S.rlen.assign((size_t)nshort, 0);
     parallel_ranges(nshort, 32768, [&](int64_t rb, int64_t re) {
         for (int64_t r = rb; r < re; ++r) {
             int64_t o = perm[(size_t)r], s = r >> 5, lane = r & 31, base = S.slice_ptr[(size_t)s];
+            S.rlen[(size_t)r] = (int32_t)(ptr[o + 1] - ptr[o]);
             for (int64_t p = ptr[o], t = 0; p < ptr[o + 1]; ++p, ++t) {
                 size_t k = (size_t)(base + t * 32 + lane);
                 S.col[k] = (int32_t)inv_other[(size_t)idx[p]];
@@ -193,6 +203,47 @@ inline void build_sell(int64_t nrows, const int64_t* ptr, const int32_t* idx, co
             if (want_src) S.lsrc[(size_t)k] = srcpos ? srcpos[p] : p;
         }
     }
+}
+
+// Byte reduction ("16-bit column deltas within slices"): a slice whose column indices span less
+// than 2^16 is NARROW -- its indices are stored as 16-bit offsets from the slice's smallest column index (cbase), 2 bytes
+// per stored entry instead of 4.  In a UC LP the rows of one period touch the variables of that period and the one
+// before (and the other way round for K'), so every slice of configs 0-3 is narrow; uniformly random columns (the
+// roofline sweep) make every slice wide and nothing changes for them.  Integer work: decoding gives back the
+// 32-bit index bit for bit.  Padding slots of a narrow slice decode to cbase (value 0.0, as before).
+inline void compress_columns(HostSell& S, bool enable) {
+    S.cbase.assign((size_t)S.nslices, -1);
+    S.col16.clear(); S.narrow_slots = 0;
+    if (!enable || S.nslices == 0) return;
+    std::vector<int64_t> narrow_of((size_t)S.nslices, 0);
+    parallel_ranges(S.nslices, 2048, [&](int64_t sb, int64_t se) {
+        for (int64_t s = sb; s < se; ++s) {
+            const int64_t b = S.slice_ptr[(size_t)s], e = S.slice_ptr[(size_t)s + 1];
+            int32_t lo = INT32_MAX, hi = -1;
+            for (int64_t lane = 0; lane < 32 && 32 * s + lane < S.nshort; ++lane)
+                for (int64_t t = 0; t < S.rlen[(size_t)(32 * s + lane)]; ++t) {
+                    const int32_t c = S.col[(size_t)(b + 32 * t + lane)];
+                    lo = std::min(lo, c); hi = std::max(hi, c);
+                }
+            if (hi < 0) { lo = 0; hi = 0; }                       // a slice of empty rows
+            if ((int64_t)hi - lo <= 65535) { S.cbase[(size_t)s] = lo; narrow_of[(size_t)s] = e - b; }
+        }
+    });
+    for (int64_t v : narrow_of) S.narrow_slots += v;
+    if (S.narrow_slots == 0) return;
+    S.col16.assign(S.col.size(), 0);
+    parallel_ranges(S.nslices, 2048, [&](int64_t sb, int64_t se) {
+        for (int64_t s = sb; s < se; ++s) {
+            const int32_t cb = S.cbase[(size_t)s];
+            if (cb < 0) continue;
+            const int64_t b = S.slice_ptr[(size_t)s];
+            for (int64_t lane = 0; lane < 32 && 32 * s + lane < S.nshort; ++lane)
+                for (int64_t t = 0; t < S.rlen[(size_t)(32 * s + lane)]; ++t) {
+                    const size_t k = (size_t)(b + 32 * t + lane);
+                    S.col16[k] = (uint16_t)(S.col[k] - cb);                 // padding slots keep offset 0
+                }
+        }
+    });
 }
 
 

@@ -60,7 +60,9 @@ struct Ctrl {
 
 struct Sell {
     const long long* sp;   // slice pointers [nslices+1]
-    const int* col;
+    const int* col;        // 32-bit column indices of the WIDE slices (NULL if every slice is narrow)
+    const unsigned short* col16;   // 16-bit offsets from cbase[slice] of the NARROW slices (NULL if every slice is wide)
+    const int* cbase;      // [nslices] >= 0: narrow slice, its smallest column index; -1: wide slice   (uc_format.hpp)
     double* val;
     long long nshort;      // rows in the sliced part
     int nslices;
@@ -100,6 +102,9 @@ __device__ __forceinline__ double ld_stream(const double* p) {   // read-once da
 }
 __device__ __forceinline__ int ld_stream(const int* p) {
     int v; asm("ld.global.nc.L1::no_allocate.s32 %0, [%1];" : "=r"(v) : "l"(p)); return v;
+}
+__device__ __forceinline__ int ld_stream(const unsigned short* p) {
+    unsigned short v; asm("ld.global.nc.L1::no_allocate.u16 %0, [%1];" : "=h"(v) : "l"(p)); return (int)v;
 }
 __device__ __forceinline__ int ld_flag(const int* p) { return *(const volatile int*)p; }
 
@@ -192,14 +197,19 @@ __device__ __forceinline__ RowId my_row(const Sell& A) { return my_row(A, (int)b
 // s[q] += sum_t val_t * g_t[q] over the entries of the row, left to right, multiply and add rounded
 // separately.  `gather(col, g)` fills g[0..NV) for a column.  Padding slots hold (col 0, val 0) and
 // add +0.0.  Sliced row: one thread, four entries' loads in flight per step.
+// column index stored at slot p of a slice whose base is cb (cb < 0: wide slice)
+__device__ __forceinline__ int sell_col(const Sell& A, int cb, long long p) {
+    return cb >= 0 ? cb + ld_stream(A.col16 + p) : ld_stream(A.col + p);
+}
 template <int NV, class G>
 __device__ __forceinline__ void sell_row(const Sell& A, int slice, int lane, double (&s)[NV], G gather) {
     long long p = __ldg(A.sp + slice) + lane;
     const long long e = __ldg(A.sp + slice + 1);
+    const int cb = __ldg(A.cbase + slice);
     for (; p + 96 < e; p += 128) {
         int c[4]; double v[4]; double g[4][NV];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) { c[u] = ld_stream(A.col + p + 32 * u); v[u] = ld_stream(A.val + p + 32 * u); }
+        for (int u = 0; u < 4; ++u) { c[u] = sell_col(A, cb, p + 32 * u); v[u] = ld_stream(A.val + p + 32 * u); }
 #pragma unroll
         for (int u = 0; u < 4; ++u) gather(c[u], g[u]);
 #pragma unroll
@@ -208,7 +218,7 @@ __device__ __forceinline__ void sell_row(const Sell& A, int slice, int lane, dou
             for (int q = 0; q < NV; ++q) s[q] = __dadd_rn(s[q], __dmul_rn(v[u], g[u][q]));
     }
     for (; p < e; p += 32) {
-        int c = ld_stream(A.col + p); double v = ld_stream(A.val + p); double g[NV];
+        int c = sell_col(A, cb, p); double v = ld_stream(A.val + p); double g[NV];
         gather(c, g);
 #pragma unroll
         for (int q = 0; q < NV; ++q) s[q] = __dadd_rn(s[q], __dmul_rn(v, g[q]));
@@ -566,7 +576,8 @@ __global__ void __launch_bounds__(kBlock) k_scale_matrix(Sell A, const double* o
     if (r.row < 0) return;
     if (r.slice >= 0) {
         const double o = r.owner ? own[r.row] : 1.0;
-        for (long long q = A.sp[r.slice] + lane; q < A.sp[r.slice + 1]; q += 32) A.val[q] = A.val[q] / (o * other[A.col[q]]);
+        const int cb = A.cbase[r.slice];
+        for (long long q = A.sp[r.slice] + lane; q < A.sp[r.slice + 1]; q += 32) A.val[q] = A.val[q] / (o * other[sell_col(A, cb, q)]);
     } else {
         const double o = own[r.row];
         for (long long q = A.lp[r.lrow] + lane; q < A.lp[r.lrow + 1]; q += 32) A.lval[q] = A.lval[q] / (o * other[A.lcol[q]]);

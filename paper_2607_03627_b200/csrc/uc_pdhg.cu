@@ -66,7 +66,7 @@ struct uc_lp {
     // one-time scalars
     double eta0 = 1.0, omega0 = 1.0, norm_b = 0.0, norm_c = 0.0;
     double precondition_seconds = 0.0, create_seconds = 0.0;
-    int64_t k_slots = 0, kt_slots = 0, k_long_nnz = 0, kt_long_nnz = 0;
+    int64_t k_slots = 0, kt_slots = 0, k_long_nnz = 0, kt_long_nnz = 0, k_narrow = 0, kt_narrow = 0;
     // step-rule factors {(k+1)^-0.6, (k+1)^-0.3}, k = 1.. (R5): a constant schedule, tabulated once
     double2* powtab = nullptr;
     long long powtab_len = 0;
@@ -118,7 +118,11 @@ Sell upload_sell(uc_lp* lp, const HostSell& H) {
     Sell S{};
     static_assert(sizeof(long long) == sizeof(int64_t), "int64 layout");
     S.sp = (const long long*)lp->upload(H.slice_ptr);
-    S.col = lp->upload(H.col);
+    // column indices: only the representation(s) that some slice uses (uc_format.hpp compress_columns)
+    const int64_t slots = (int64_t)H.col.size();
+    S.col = H.narrow_slots < slots ? lp->upload(H.col) : nullptr;
+    S.col16 = H.narrow_slots > 0 ? lp->upload(H.col16) : nullptr;
+    S.cbase = lp->upload(H.cbase);
     S.val = lp->upload(H.val);
     S.nshort = H.nshort; S.nslices = (int)H.nslices; S.nblk = cdiv(H.nslices, kWarps);
     S.lp = (const long long*)lp->upload(H.lptr);
@@ -212,17 +216,17 @@ void grow_powtab(uc_lp* lp, long long need, long long limit, cudaStream_t st, st
 // (griddepcontrol.wait) before it reads anything a previous kernel wrote.  Captured into the graph as
 // programmatic dependency edges.
 template <class Kern>
-void launch_pdl(Kern kern, int grid, size_t smem, cudaStream_t st, const Sell& A, const Vecs& V, Ctrl* ctl) {
+void launch_pdl(Kern kern, int grid, int threads, size_t smem, cudaStream_t st, const Sell& A, const Vecs& V, Ctrl* ctl) {
     cudaLaunchConfig_t cfg{};
-    cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3(kAttemptThreads); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3((unsigned)threads); cfg.dynamicSmemBytes = smem; cfg.stream = st;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
     CK(cudaLaunchKernelEx(&cfg, kern, A, V, ctl));
 }
-void launch_primal(uc_lp* lp, cudaStream_t st) { launch_pdl(k_primal, lp->V.gridPA, sizeof(PrimalSmem), st, lp->KT, lp->V, lp->ctl); }
-void launch_dual(uc_lp* lp, cudaStream_t st) { launch_pdl(k_dual, lp->V.gridPB, sizeof(DualSmem), st, lp->K, lp->V, lp->ctl); }
+void launch_primal(uc_lp* lp, cudaStream_t st) { launch_pdl(k_primal, lp->V.gridPA, kPrimalThreads, kPrimalSmemBytes, st, lp->KT, lp->V, lp->ctl); }
+void launch_dual(uc_lp* lp, cudaStream_t st) { launch_pdl(k_dual, lp->V.gridPB, kDualThreads, kDualSmemBytes, st, lp->K, lp->V, lp->ctl); }
 void launch_attempt(uc_lp* lp, cudaStream_t st) { launch_primal(lp, st); launch_dual(lp, st); }
 void launch_kkt(uc_lp* lp, cudaStream_t st, int mode) {
     const int flush = mode == kModeCheck;        // the periodic check also applies the pending average term (R6)
@@ -288,10 +292,11 @@ void destroy_impl(uc_lp* lp) {
 }
 
 int64_t bytes_per_attempt(const uc_lp* lp) {
-    // what one attempt streams in THIS layout: matrix slots (12 B each, padding included),
-    // step descriptors (8 B per scheduled step, padding steps included), and per variable 8 (x) + 24 (c,l,u) + 16 (xsum r/w) + 8 (x') + 16 ({xbar,dx}) + 16
+    // what one attempt streams in THIS layout: matrix slots (8 B value + 4 B index, or 2 B index in a narrow
+    // slice; padding included), step descriptors (16 B per scheduled step, padding steps included), and per variable 8 (x) + 24 (c,l,u) + 16 (xsum r/w) + 8 (x') + 16 ({xbar,dx}) + 16
     // (gather of the pair) = 88 B, per row 8 (y) + 8 (q) + 1 (sense) + 16 (ysum r/w) + 8 (y') + 8 (gather) = 49 B
-    return 12 * (lp->k_slots + lp->kt_slots + lp->k_long_nnz + lp->kt_long_nnz) + 8 * ((int64_t)lp->K.steps_per_warp * lp->K.sched_warps + (int64_t)lp->KT.steps_per_warp * lp->KT.sched_warps) +
+    return 12 * (lp->k_slots + lp->kt_slots + lp->k_long_nnz + lp->kt_long_nnz) - 2 * (lp->k_narrow + lp->kt_narrow) +
+           16 * ((int64_t)lp->K.steps_per_warp * lp->K.sched_warps + (int64_t)lp->KT.steps_per_warp * lp->KT.sched_warps) +
            88 * lp->n + 49 * lp->m;
 }
 
@@ -314,6 +319,8 @@ int uc_host_layout_selftest(int64_t m, int64_t n, int64_t nnz, const int64_t* ro
     build_perms(m, n, nnz, row_ptr, col_idx, sell_window, long_row_threshold, P);
     build_K(row_ptr, col_idx, val, true, P);
     build_KT(row_ptr, col_idx, val, true, P);
+    compress_columns(P.K, true);
+    compress_columns(P.KT, true);
     build_schedule(P.K, sched_warps);
     build_schedule(P.KT, sched_warps);
     auto bad = [&](const std::string& what) { return fail(UC_ERR_INVALID, what); };
@@ -380,6 +387,25 @@ int uc_host_layout_selftest(int64_t m, int64_t n, int64_t nnz, const int64_t* ro
                 if (S.lcol[k] != (int32_t)c_new || std::memcmp(&S.lval[k], &v, sizeof v) != 0 || S.lsrc[k] != pos) return "long row entry";
             }
         }
+        // ---- 16-bit column offsets: a narrow slice decodes to the 32-bit indices bit for bit, its span fits 16 bits,
+        // and a slice is wide only if its span does not fit
+        if ((int64_t)S.cbase.size() != S.nslices) return "cbase size";
+        for (int64_t s = 0; s < S.nslices; ++s) {
+            const int32_t cb = S.cbase[(size_t)s];
+            int32_t lo = INT32_MAX, hi = -1;
+            for (int64_t lane = 0; lane < 32 && 32 * s + lane < S.nshort; ++lane) {
+                const int64_t len = row_len(perm[(size_t)(32 * s + lane)]);
+                for (int64_t t = 0; t < len; ++t) {
+                    const size_t k = (size_t)(S.slice_ptr[(size_t)s] + 32 * t + lane);
+                    lo = std::min(lo, S.col[k]); hi = std::max(hi, S.col[k]);
+                    if (cb >= 0 && cb + (int32_t)S.col16[k] != S.col[k]) return "16-bit column offset does not decode to the index";
+                }
+            }
+            if (hi >= 0) {
+                if (cb >= 0 && (cb != lo || hi - lo > 65535)) return "narrow slice base / span";
+                if (cb < 0 && (int64_t)hi - lo <= 65535) return "a slice that fits 16 bits is stored wide";
+            }
+        }
         // ---- schedule: every slice exactly once, as consecutive chunks of one warp, flags and offsets right
         const int64_t W = S.sched_warps, J = S.steps_per_warp;
         if ((int64_t)S.steps.size() != W * J) return "schedule size";
@@ -389,7 +415,7 @@ int uc_host_layout_selftest(int64_t m, int64_t n, int64_t nnz, const int64_t* ro
             for (int64_t j = 0; j < J; ) {
                 const StepDesc d = S.steps[(size_t)(j * W + wq)];
                 const uint32_t info = d.w0 >> 26;
-                if (ended) { if (d.w0 != 0 || d.row0 != 0) return "step after the end marker"; ++j; continue; }
+                if (ended) { if (d.w0 != 0 || d.row0 != 0 || d.cbase != -1) return "step after the end marker"; ++j; continue; }
                 if (info & kStepEnd) { if ((info & 31) != 0) return "end marker carries work"; ended = true; ++j; continue; }
                 if (!(info & kStepFirst) || d.row0 % 32) return "slice does not start with its first chunk";
                 const int64_t sl = d.row0 / 32;
@@ -403,7 +429,7 @@ int uc_host_layout_selftest(int64_t m, int64_t n, int64_t nnz, const int64_t* ro
                     const StepDesc e = S.steps[(size_t)(j * W + wq)];
                     const uint32_t ei = e.w0 >> 26;
                     const int64_t nt = std::max<int64_t>(0, std::min<int64_t>(kChunkT, wd - kChunkT * c));
-                    if (e.row0 != d.row0 || (int64_t)(ei & 7) != nt || ((ei & kStepFirst) != 0) != (c == 0) ||
+                    if (e.row0 != d.row0 || e.cbase != S.cbase[(size_t)sl] || (int64_t)(ei & 7) != nt || ((ei & kStepFirst) != 0) != (c == 0) ||
                         ((ei & kStepLast) != 0) != (c == nch - 1) || (ei & kStepEnd) ||
                         ((int64_t)(e.w0 & 0x3ffffffu) << 5) != S.slice_ptr[(size_t)sl] + 32 * kChunkT * c)
                         return "chunk descriptor";
@@ -430,7 +456,7 @@ double uc_host_exp_rounded(double x) { return exp_rounded(x); }
 void uc_lp_default_options(uc_lp_options* o) {
     if (!o) return;
     o->device = -1; o->ruiz_iters = 10; o->pc_alpha = 1.0; o->sell_window = 4096; o->long_row_threshold = 32;
-    o->keep_source_map = 0; o->pad_ = 0;
+    o->keep_source_map = 0; o->index_compression = 1;
 }
 
 void uc_pdhg_default_params(uc_pdhg_params* p) {
@@ -484,8 +510,8 @@ int uc_lp_create(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, cons
             CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
             const int cap = kCtasPerSm * std::max(sms, 1);
             const int64_t sl_kt = (P.nshort_c + 31) / 32, sl_k = (P.nshort_r + 31) / 32;
-            gridPA = (int)std::max<int64_t>(1, std::min<int64_t>(cap, std::max<int64_t>((sl_kt + kAttWarps - 1) / kAttWarps, n - P.nshort_c)));
-            gridPB = (int)std::max<int64_t>(1, std::min<int64_t>(cap, std::max<int64_t>((sl_k + kAttWarps - 1) / kAttWarps, m - P.nshort_r)));
+            gridPA = (int)std::max<int64_t>(1, std::min<int64_t>(cap, std::max<int64_t>((sl_kt + kPrimalWarps - 1) / kPrimalWarps, n - P.nshort_c)));
+            gridPB = (int)std::max<int64_t>(1, std::min<int64_t>(cap, std::max<int64_t>((sl_k + kDualWarps - 1) / kDualWarps, m - P.nshort_r)));
         }
         const bool want_src = opt.keep_source_map != 0;
         std::exception_ptr k_side_error;
@@ -494,20 +520,23 @@ int uc_lp_create(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, cons
                 cudaSetDevice(dev);
                 build_K(row_ptr, col_idx, val, want_src, P);
                 if (P.K.col.size() >= (size_t)1 << 31) throw std::bad_alloc();   // step descriptors address entries / 32 in 26 bits
-                build_schedule(P.K, (int64_t)gridPB * kAttWarps);
+                compress_columns(P.K, opt.index_compression != 0);
+                build_schedule(P.K, (int64_t)gridPB * kDualWarps);
                 lp->K = upload_sell(lp, P.K);
             } catch (...) { k_side_error = std::current_exception(); }
         });
         try {
             build_KT(row_ptr, col_idx, val, want_src, P);
             if (P.KT.col.size() >= (size_t)1 << 31) throw std::bad_alloc();
-            build_schedule(P.KT, (int64_t)gridPA * kAttWarps);
+            compress_columns(P.KT, opt.index_compression != 0);
+            build_schedule(P.KT, (int64_t)gridPA * kPrimalWarps);
             lp->KT = upload_sell(lp, P.KT);
         } catch (...) { k_side.join(); throw; }
         k_side.join();
         if (k_side_error) std::rethrow_exception(k_side_error);
         lp->k_slots = (int64_t)P.K.col.size(); lp->kt_slots = (int64_t)P.KT.col.size();
         lp->k_long_nnz = (int64_t)P.K.lcol.size(); lp->kt_long_nnz = (int64_t)P.KT.lcol.size();
+        lp->k_narrow = P.K.narrow_slots; lp->kt_narrow = P.KT.narrow_slots;
         lp->perm_r = (long long*)lp->upload(P.perm_r);
         lp->perm_c = (long long*)lp->upload(P.perm_c);
         lp->h_perm_r = P.perm_r; lp->h_perm_c = P.perm_c;
@@ -531,8 +560,8 @@ int uc_lp_create(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, cons
             V.gridA = std::max(1, std::min(cap, lp->KT.grid)); V.gridB = std::max(1, std::min(cap, lp->K.grid));
         }
         V.gridPA = gridPA; V.gridPB = gridPB;
-        CK(cudaFuncSetAttribute(k_primal, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(PrimalSmem)));
-        CK(cudaFuncSetAttribute(k_dual, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(DualSmem)));
+        CK(cudaFuncSetAttribute(k_primal, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kPrimalSmemBytes));
+        CK(cudaFuncSetAttribute(k_dual, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kDualSmemBytes));
         V.partA = lp->dalloc<dd>((size_t)V.gridPA);
         V.partB = lp->dalloc<dd>((size_t)2 * V.gridPB);
         V.partD = lp->dalloc<dd>((size_t)8 * V.gridA);
@@ -824,6 +853,7 @@ int uc_lp_get_info(const uc_lp* lp, uc_lp_info* info) {
     info->precondition_seconds = lp->precondition_seconds; info->create_seconds = lp->create_seconds;
     info->eta0 = lp->eta0; info->omega0 = lp->omega0; info->norm_b = lp->norm_b; info->norm_c = lp->norm_c;
     info->bytes_per_attempt = bytes_per_attempt(lp);
+    info->k_narrow_slots = lp->k_narrow; info->kt_narrow_slots = lp->kt_narrow;
     return UC_OK;
 }
 

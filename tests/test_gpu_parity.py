@@ -142,6 +142,36 @@ def test_trajectory_parity_is_layout_independent(window, thr):
     assert_trajectory_parity(get_lp("ragged"), 130, sell_window=window, long_row_threshold=thr)
 
 
+@pytest.mark.parametrize("name", ["uc1", "ragged", "random_2e4"])
+def test_index_compression_is_bit_identical(name):
+    """SURVEY.md 8(f) NEXT-4, 16-bit column offsets inside a slice: integer work, so the iterates with and without it are
+    the same bits (and both match the oracle through test_trajectory_parity_200_attempts)."""
+    lp = get_lp(name)
+    with P.UcLp(lp, index_compression=1) as h:
+        a = h.solve(fixed_iterations=300)
+        ia = h.info()
+    with P.UcLp(lp, index_compression=0) as h:
+        b = h.solve(fixed_iterations=300)
+        ib = h.info()
+    np.testing.assert_array_equal(a.x, b.x); np.testing.assert_array_equal(a.y, b.y)
+    assert ib.k_narrow_slots == ib.kt_narrow_slots == 0
+    assert ib.bytes_per_attempt - ia.bytes_per_attempt == 2 * (ia.k_narrow_slots + ia.kt_narrow_slots)
+    if name == "uc1":       # period-local structure: every slice of K is narrow; in K' the reserve columns reach the long
+        assert ia.k_narrow_slots == ia.k_sell_slots         # reserve rows, which sit at the end of the permuted row space
+        assert 0.95 * ia.kt_sell_slots <= ia.kt_narrow_slots <= ia.kt_sell_slots
+
+
+def test_index_compression_mixed_narrow_and_wide_slices():
+    from test_layout_cpu import banded_and_wide_lp
+    lp = banded_and_wide_lp()
+    so = oracle.solve(lp, fixed_iterations=130)
+    with P.UcLp(lp) as h:
+        sg = h.solve(fixed_iterations=130)
+        i = h.info()
+    assert 0 < i.k_narrow_slots < i.k_sell_slots
+    assert rel_l2(sg.x, so.x) <= TOL_ITER and rel_l2(sg.y, so.y) <= TOL_ITER
+
+
 def test_trajectory_parity_other_check_period_and_tail():
     lp = get_lp("uc0")
     for F, ce in ((37, 10), (64, 64), (65, 64), (1, 64)):

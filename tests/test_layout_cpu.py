@@ -29,6 +29,36 @@ def test_layout_options_and_warp_counts(window, thr, warps):
         B.host_layout_selftest(lp, sell_window=window, long_row_threshold=thr, sched_warps=warps)
 
 
+def banded_and_wide_lp(n=200_000, m=150_000, seed=4):
+    """Rows whose columns lie in a narrow band (16-bit offsets apply) mixed with rows that reach across all 200,000
+    columns (slices that stay 32-bit), plus one explicit zero at column 0 (must not be mistaken for padding)."""
+    from workloads.lp import from_coo
+    rng = np.random.default_rng(seed)
+    rows, cols = [], []
+    for i in range(m):
+        if i % 3000 < 2900:                                        # banded rows
+            c = (i * n) // m + rng.choice(2000, size=3, replace=False)
+        else:                                                      # wide rows
+            c = rng.choice(n, size=4, replace=False)
+        c = np.unique(np.clip(c, 0, n - 1))
+        rows += [i] * len(c); cols += c.tolist()
+    vals = rng.standard_normal(len(rows))
+    if cols[0] != 0:
+        rows.insert(0, 0); cols.insert(0, 0); vals = np.concatenate([[0.0], vals])
+    else:
+        vals[0] = 0.0
+    return from_coo(m, n, rows, cols, vals, np.full(m, ord("G"), np.uint8), np.zeros(m), rng.standard_normal(n),
+                    -np.ones(n), np.ones(n), name="banded_and_wide")
+
+
+def test_sixteen_bit_column_offsets_on_narrow_and_wide_slices():
+    """the self-check decodes every narrow slice back to its 32-bit indices, and checks that a
+    slice is wide only when its span does not fit 16 bits -- on an LP that has both kinds."""
+    lp = banded_and_wide_lp()
+    B.host_layout_selftest(lp)
+    B.host_layout_selftest(lp, sell_window=64, long_row_threshold=3)
+
+
 def test_degenerate_shapes():
     z = np.zeros(0)
     empty = LP(m=0, n=0, row_ptr=np.zeros(1, np.int64), col_idx=np.zeros(0, np.int32), val=z, sense=np.zeros(0, np.uint8),
