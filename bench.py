@@ -33,17 +33,29 @@ METRIC = "pdhg_attempts_per_s"
 UNIT = "attempts/s"
 
 
-def algorithmic_bytes(m, n, nnz):
+def algorithmic_bytes(m, n, nnz, info=None):
     """bytes one attempt must move (fp64 values, int32 indices, both matrix copies, every
-    vector once, gathers counted once).  Split by kernel; the sum is 24 nnz + 76 n + 53 m + 8."""
-    primal = 12 * nnz + 4 * (n + 1) + 64 * n + 8 * m       # K' pass: matrix, ptr, x c l u (32) + x' xbar (16) + xsum r/w (16), gather of y
-    dual = 12 * nnz + 4 * (m + 1) + 41 * m + 8 * n         # K pass: matrix, ptr, y q sense (17) + y' (8) + ysum r/w (16), gather of xbar
-    return primal, dual
+    vector once, gathers counted once).  Split by kernel; the sum is 24 nnz + 76 n + 53 m + 8.
+    With `info` (uc_lp_get_info) the index bytes are those of THIS layout: 2 instead of 4 per entry in the slices that
+    store 16-bit column offsets ("never credit bytes that were not moved")."""
+    idx_kt = idx_k = 4.0
+    if info is not None:
+        idx_kt = 4.0 - 2.0 * info.kt_narrow_slots / max(info.kt_sell_slots + info.kt_long_nnz, 1)
+        idx_k = 4.0 - 2.0 * info.k_narrow_slots / max(info.k_sell_slots + info.k_long_nnz, 1)
+    primal = (8 + idx_kt) * nnz + 4 * (n + 1) + 64 * n + 8 * m     # K' pass: matrix, ptr, x c l u (32) + x' xbar (16) + xsum r/w (16), gather of y
+    dual = (8 + idx_k) * nnz + 4 * (m + 1) + 41 * m + 8 * n        # K pass: matrix, ptr, y q sense (17) + y' (8) + ysum r/w (16), gather of xbar
+    return int(primal), int(dual)
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the attempt kernels on config 3, from the one
-# `ncu --set full` capture summarised in profiles/r01d_summary.md (cold L2 per replay; bytes)
-NCU_TRAFFIC_CONFIG3 = {"k_primal": 185.04e6 + 14.06e6, "k_dual": 161.37e6 + 4.17e6, "source": "profiles/r01d_summary.md"}
+def ncu_traffic(config):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the attempt kernels, from the tracked artefact that the
+    ncu summary of the same capture is written with (profiles/r02_traffic.json; bytes; cold L2 per replay)."""
+    p = os.path.join(ROOT, "profiles", "r02_traffic.json")
+    try:
+        d = json.load(open(p))
+        return d.get(f"uc_config{config}"), "profiles/r02_traffic.json"
+    except Exception:
+        return None, None
 
 
 def load_peaks():
@@ -154,20 +166,23 @@ def aggregate(local_seconds, local_units, dist=None, device=None):
     return float(t.item()), float(u.item())
 
 
-def all_configs_table(handles=(1, 2, 3)):
-    """--all-configs: one markdown table over BASELINE.json's configs (UC 0-3, roofline sweep seeds 10-13): attempts/s of
-    `uc_pdhg_solve_device` with fixed attempts (CUDA-event loop time), and the aggregate rate of concurrent handles
-    on the latency-bound config 1.  Reporting only: the bench line of the contract is the default run."""
-    import threading
+def all_configs_table(batch_sizes=(1, 4, 16, 45)):
+    """--all-configs: markdown tables over BASELINE.json's configs (UC 0-3; roofline sweep seeds 10-14 at the 200 fixed
+    attempts north_star states) plus the tuned-presolve shape of PAPER.md Table VII: attempts/s of `uc_pdhg_solve_device`
+    (CUDA-event loop time, checks and restarts included), and the aggregate rate of `uc_pdhg_solve_batch` on the
+    launch-latency-bound LPs (the paper's 45 scenarios, P:l.101).  Reporting only: the bench line of the contract is the
+    default run."""
+    import numpy as np
     import torch
     import paper_2607_03627_b200 as P
     from workloads import sweep_config, uc_config
     peak, _ = load_peaks()
     st = torch.cuda.Stream()
-    print("| workload | m | n | nnz | us/attempt (in graph, checks incl.) | attempts/s | algorithmic MB/attempt | GB/s | % of measured peak | device MB | create ms |")
-    print("|---|---|---|---|---|---|---|---|---|---|---|")
+    print("| workload | m | n | nnz | attempts | us/attempt (in graph, checks incl.) | attempts/s | algorithmic MB/attempt (this layout / 32-bit indices) | GB/s | % of measured peak | 16-bit-offset slots % | device MB | create ms |")
+    print("|---|---|---|---|---|---|---|---|---|---|---|---|---|")
     cases = [(f"UC config {c}", (lambda c=c: uc_config(c)), 2048) for c in (0, 1, 2, 3)]
-    cases += [(f"config 4, seed {s_}", (lambda s_=s_: sweep_config(s_)), 200 if s_ < 13 else 64) for s_ in (10, 11, 12, 13)]
+    cases += [("UC tuned-presolve shape (P: Table VII)", (lambda: uc_config("tuned_presolve")), 2048)]
+    cases += [(f"config 4, seed {s_}", (lambda s_=s_: sweep_config(s_)), 200) for s_ in (10, 11, 12, 13, 14)]
     for name, make, attempts in cases:
         lp = make()
         t = time.perf_counter(); h = P.UcLp(lp, device=0); tc = time.perf_counter() - t
@@ -175,29 +190,29 @@ def all_configs_table(handles=(1, 2, 3)):
         for _ in range(2):
             r = h.solve_device(x, y, fixed_iterations=attempts, stream=st.cuda_stream)
         us = r.loop_seconds * 1e6 / attempts
-        bp, bd = algorithmic_bytes(lp.m, lp.n, lp.nnz)
-        print(f"| {name} | {lp.m} | {lp.n} | {lp.nnz} | {us:.2f} | {1e6 / us:.0f} | {(bp + bd) / 1e6:.1f} | {(bp + bd) / us / 1e3:.0f} | "
-              f"{(bp + bd) / us / 1e3 / peak * 100:.1f} | {h.info().device_bytes / 1e6:.0f} | {tc * 1e3:.0f} |", flush=True)
+        i = h.info()
+        bp, bd = algorithmic_bytes(lp.m, lp.n, lp.nnz, i)
+        sp, sd = algorithmic_bytes(lp.m, lp.n, lp.nnz)
+        narrow = 100.0 * (i.k_narrow_slots + i.kt_narrow_slots) / max(i.k_sell_slots + i.kt_sell_slots, 1)
+        print(f"| {name} | {lp.m} | {lp.n} | {lp.nnz} | {attempts} | {us:.2f} | {1e6 / us:.0f} | {(bp + bd) / 1e6:.1f} / {(sp + sd) / 1e6:.1f} | "
+              f"{(bp + bd) / us / 1e3:.0f} | {(bp + bd) / us / 1e3 / peak * 100:.1f} | {narrow:.0f} | {i.device_bytes / 1e6:.0f} | {tc * 1e3:.0f} |", flush=True)
         h.close()
+        del lp, x, y
     print()
-    print("| config | concurrent handles (one thread and one stream each) | aggregate attempts/s | results identical |")
-    print("|---|---|---|---|")
-    lp = uc_config(1)
-    for nh in handles:
-        hs = [P.UcLp(lp, device=0) for _ in range(nh)]
-        sts = [torch.cuda.Stream() for _ in range(nh)]
-        xs = [torch.empty(lp.n, dtype=torch.float64, device="cuda") for _ in range(nh)]
-        ys = [torch.empty(lp.m, dtype=torch.float64, device="cuda") for _ in range(nh)]
-
-        def run(i):
-            hs[i].solve_device(xs[i], ys[i], fixed_iterations=2048, stream=sts[i].cuda_stream)
-        for _ in range(2):
-            th = [threading.Thread(target=run, args=(i,)) for i in range(nh)]
-            torch.cuda.synchronize(); t = time.perf_counter()
-            [t_.start() for t_ in th]; [t_.join() for t_ in th]
-            torch.cuda.synchronize(); dt = time.perf_counter() - t
-        same = all(torch.equal(xs[0], xs[i]) for i in range(1, nh))
-        print(f"| 1 | {nh} | {nh * 2048 / dt:.0f} | {same} |", flush=True)
+    print("| workload | LPs in one uc_pdhg_solve_batch call (16 in flight) | aggregate attempts/s | per-LP attempts/s | results identical to a solo solve |")
+    print("|---|---|---|---|---|")
+    for name, key in (("UC config 0", 0), ("UC tuned-presolve shape", "tuned_presolve"), ("UC config 1", 1)):
+        lp = uc_config(key)
+        F = 2048
+        hs = [P.UcLp(lp, device=0) for _ in range(max(batch_sizes))]
+        solo = hs[0].solve(fixed_iterations=F)
+        for nb in batch_sizes:
+            for _ in range(2):
+                torch.cuda.synchronize(); t = time.perf_counter()
+                out = P.solve_batch(hs[:nb], fixed_iterations=F)
+                dt = time.perf_counter() - t
+            same = all(np.array_equal(o.x, solo.x) and np.array_equal(o.y, solo.y) for o in out)
+            print(f"| {name} | {nb} | {nb * F / dt:.0f} | {F / dt:.0f} | {same} |", flush=True)
         for h in hs:
             h.close()
 
@@ -277,17 +292,25 @@ def main():
     out = None
     if rank == 0:
         peak, peak_src = load_peaks()
-        bp, bd = algorithmic_bytes(lp.m, lp.n, lp.nnz)
+        bp, bd = algorithmic_bytes(lp.m, lp.n, lp.nnz, info)          # what this layout moves (16-bit offsets counted as 2 B)
+        sp, sd = algorithmic_bytes(lp.m, lp.n, lp.nnz)                # SURVEY.md 8(d) formula with 32-bit indices everywhere
         dom = ("k_primal", bp, primal_ms) if primal_ms >= dual_ms else ("k_dual", bd, dual_ms)
         ach = dom[1] / (dom[2] * 1e-3) / 1e9
         att_ms = 1e3 * loop_s / (args.steps * A)
+        traffic, traffic_src = ncu_traffic(args.config)
+        tr = traffic.get(dom[0]) if traffic else None
         roof = {"bound": "hbm", "kernel": dom[0], "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                "traffic": NCU_TRAFFIC_CONFIG3[dom[0]] if args.config == 3 else None,
-                "traffic_source": NCU_TRAFFIC_CONFIG3["source"] if args.config == 3 else None, "peak_source": peak_src, "algorithmic_bytes_per_launch": dom[1], "kernel_ms": dom[2],
+                "what": "effective bandwidth: ALGORITHMIC bytes of the kernel / its CUDA-event time; frac_dram is the same with the "
+                        "DRAM bytes ncu measured (gathers served from L2 are not DRAM traffic)",
+                "traffic": tr, "traffic_source": traffic_src if tr else None,
+                "frac_dram": (tr / (dom[2] * 1e-3) / 1e9 / peak) if tr else None,
+                "peak_source": peak_src, "algorithmic_bytes_per_launch": dom[1], "kernel_ms": dom[2],
                 "other_kernel": {"k_primal_ms": primal_ms, "k_dual_ms": dual_ms, "k_primal_bytes": bp, "k_dual_bytes": bd},
-                "attempt": {"algorithmic_bytes": bp + bd, "ms_in_graph": att_ms, "GB/s": (bp + bd) / (att_ms * 1e-3) / 1e9,
+                "attempt": {"algorithmic_bytes": bp + bd, "algorithmic_bytes_32bit_indices": sp + sd, "ms_in_graph": att_ms,
+                            "GB/s": (bp + bd) / (att_ms * 1e-3) / 1e9,
                             "frac_of_peak": (bp + bd) / (att_ms * 1e-3) / 1e9 / peak,
                             "frac_of_8TBs": (bp + bd) / (att_ms * 1e-3) / 1e9 / 8000.0,
+                            "frac_of_8TBs_32bit_formula": (sp + sd) / (att_ms * 1e-3) / 1e9 / 8000.0,
                             "layout_bytes": int(info.bytes_per_attempt)}}
         # ---- e2e: host CSR -> create -> solve to rel KKT 1e-4 -> x, y in host memory
         h2d = lp.row_ptr.nbytes + lp.col_idx.nbytes + lp.val.nbytes + lp.sense.nbytes + lp.b.nbytes + lp.c.nbytes + lp.l.nbytes + lp.u.nbytes

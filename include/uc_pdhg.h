@@ -87,6 +87,12 @@ int uc_lp_create(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, cons
    matrix, its scalings and the captured graph are kept.  l_new/u_new: host, length n. */
 int uc_lp_update_bounds(uc_lp* lp, const double* l_new, const double* u_new);
 
+/* Replace the objective (re-solves inside branch-and-bound and cost sweeps):
+   c~ = c / D_c is rescaled with the scalings already on the device, ||c|| (R9) and omega0 = ||c~|| / ||q~|| (R2)
+   are recomputed; the matrix, its scalings and the captured graph are kept.  c_new: host, length n, finite.
+   The handle then behaves exactly like one created with c_new (the preconditioner does not depend on c). */
+int uc_lp_update_objective(uc_lp* lp, const double* c_new);
+
 void uc_lp_destroy(uc_lp* lp); /* NULL ok; must not race with a solve on the same handle */
 
 /* ------------------------------------------------------------------------------------------- solve */
@@ -149,6 +155,16 @@ int uc_pdhg_solve(uc_lp* lp, const uc_pdhg_params* params, double* x_out, double
    (the torch harness owns them); nothing but the result struct and the traces crosses PCIe. */
 int uc_pdhg_solve_device(uc_lp* lp, const uc_pdhg_params* params, double* x_out_device, double* y_out_device,
                          uc_pdhg_result* result);
+
+/* Batched solve of independent LPs (the paper's 45 scenarios): solves
+   handles[0..count) concurrently, each on its own handle's stream, with up to max_concurrent (<= 0: 16) solves in
+   flight, and returns when all are done.  Small LPs are bound by the two dependent kernel launches of an attempt
+   (~6-8 us each), not by the GPU: solves in flight at the same time fill it.  Every result is bit-identical to the
+   solve run alone.  params: one set for all (NULL = defaults); its stream / x0 / y0 / trace fields must be NULL.
+   x_out[i] / y_out[i]: HOST buffers of handle i (the arrays or any entry may be NULL).  results[count].
+   Returns 0, or the first failure (uc_last_error names the solve); uc_pdhg_cancel(handles[i]) stops solve i. */
+int uc_pdhg_solve_batch(uc_lp* const* handles, int32_t count, const uc_pdhg_params* params, double* const* x_out,
+                        double* const* y_out, uc_pdhg_result* results, int32_t max_concurrent);
 
 /* Cancel, any thread, idempotent (Algorithm 1: "Terminate the other solver").
    - A solve is in flight on the handle: THAT solve returns UC_CANCELLED at its next check (within one check

@@ -59,8 +59,8 @@ ATTEMPT_DTYPE = np.dtype([("eta_used", "f8"), ("eta_bar", "f8"), ("eta_next", "f
 CHECK_DTYPE = np.dtype([("k", "i8"), ("restart_kind", "i4"), ("candidate", "i4"), ("omega_after", "f8"),
                         ("mu_c", "f8"), ("mu_r", "f8"), ("relkkt_cur", "f8"), ("relkkt_avg", "f8")])
 
-EXPORTS = ["uc_lp_default_options", "uc_lp_create", "uc_lp_update_bounds", "uc_lp_destroy",
-           "uc_pdhg_default_params", "uc_pdhg_solve", "uc_pdhg_solve_device", "uc_pdhg_cancel", "uc_pdhg_time_kernels",
+EXPORTS = ["uc_lp_default_options", "uc_lp_create", "uc_lp_update_bounds", "uc_lp_update_objective", "uc_lp_destroy",
+           "uc_pdhg_default_params", "uc_pdhg_solve", "uc_pdhg_solve_device", "uc_pdhg_solve_batch", "uc_pdhg_cancel", "uc_pdhg_time_kernels",
            "uc_lp_get_info", "uc_lp_get_scaling", "uc_lp_get_scaled_values", "uc_lp_spmv", "uc_last_error",
            "uc_host_log_rounded", "uc_host_exp_rounded", "uc_host_layout_selftest"]
 
@@ -93,8 +93,10 @@ def load_library(build_if_missing: bool = True):
     lib.uc_pdhg_cancel.argtypes = [C.c_void_p]
     lib.uc_lp_create.argtypes = [C.c_int64, C.c_int64, C.c_int64] + [C.c_void_p] * 10
     lib.uc_lp_update_bounds.argtypes = [C.c_void_p] * 3
+    lib.uc_lp_update_objective.argtypes = [C.c_void_p] * 2
     lib.uc_pdhg_solve.argtypes = [C.c_void_p] * 5
     lib.uc_pdhg_solve_device.argtypes = [C.c_void_p] * 5
+    lib.uc_pdhg_solve_batch.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32]
     lib.uc_pdhg_time_kernels.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
     lib.uc_host_layout_selftest.argtypes = [C.c_int64, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p,
                                             C.c_int32, C.c_int32, C.c_int32]
@@ -167,6 +169,24 @@ class Solution:
     checks: np.ndarray
 
 
+def solve_batch(handles, max_concurrent=0, want_xy=True, **params):
+    """uc_pdhg_solve_batch: solve the LPs of `handles` (UcLp objects) concurrently; returns one Solution per handle."""
+    lib = load_library()
+    k = len(handles)
+    prm = default_params(**params)
+    hs = (C.c_void_p * k)(*[h._h for h in handles])
+    xs = [np.zeros(h.n) if want_xy else None for h in handles]
+    ys = [np.zeros(h.m) if want_xy else None for h in handles]
+    px = (C.c_void_p * k)(*[C.c_void_p(x.ctypes.data) if want_xy and x.size else None for x in xs]) if want_xy else None
+    py = (C.c_void_p * k)(*[C.c_void_p(y.ctypes.data) if want_xy and y.size else None for y in ys]) if want_xy else None
+    res = (Result * k)()
+    _check(lib.uc_pdhg_solve_batch(C.cast(hs, C.c_void_p), k, C.cast(C.byref(prm), C.c_void_p),
+                                   C.cast(px, C.c_void_p) if want_xy else None, C.cast(py, C.c_void_p) if want_xy else None,
+                                   C.cast(res, C.c_void_p), int(max_concurrent)))
+    empty_a, empty_c = np.zeros(0, dtype=ATTEMPT_DTYPE), np.zeros(0, dtype=CHECK_DTYPE)
+    return [UcLp._solution(res[i], xs[i], ys[i], empty_a, empty_c, 0, 0) for i in range(k)]
+
+
 class UcLp:
     """Owner of one uc_lp handle.  `lp` is any object with m, n, row_ptr, col_idx, val, sense, b, c, l, u."""
 
@@ -212,6 +232,13 @@ class UcLp:
         _check(self.lib.uc_lp_update_bounds(self._h, lp_, up_))
 
     update_bounds = uc_lp_update_bounds
+
+    def uc_lp_update_objective(self, c):
+        ca, cp = _host(c, np.float64)
+        assert ca.shape == (self.n,)
+        _check(self.lib.uc_lp_update_objective(self._h, cp))
+
+    update_objective = uc_lp_update_objective
 
     def uc_pdhg_time_kernels(self, attempts=64, stream=None):
         """(primal_ms, dual_ms): average device time of the two kernels of an attempt (CUDA events)."""

@@ -89,6 +89,22 @@ __device__ __forceinline__ void cp_gather(double* dst, const double* src) {
 __device__ __forceinline__ void cp_gather(double2* dst, const double2* src) {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"(src) : "memory");   // L1 bypass: measured faster
 }
+// Predicated forms: `on` becomes a predicate on the copy itself.  The conditions below are warp-uniform functions of
+// the step descriptor, but the compiler cannot know that (the descriptor comes out of a shuffle), so an `if` around a
+// copy costs a BSSY / BRA / BSYNC triple; ncu showed control flow at 21 % of the instructions of the loop, which is
+// bound by instruction issue latency at 4 warps per scheduler (profiles/r02a).
+__device__ __forceinline__ void cp_stream16_if(bool on, void* dst, const void* src, uint64_t pol) {
+    asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.s32 q, %0, 0;\n\t@q cp.async.cg.shared.global.L2::cache_hint [%1], [%2], 16, %3;\n\t}"
+                 ::"r"((int)on), "r"(smem_u32(dst)), "l"(src), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void cp_gather_if(bool on, double* dst, const double* src) {
+    asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.s32 q, %0, 0;\n\t@q cp.async.ca.shared.global [%1], [%2], 8;\n\t}"
+                 ::"r"((int)on), "r"(smem_u32(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_gather_if(bool on, double2* dst, const double2* src) {
+    asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.s32 q, %0, 0;\n\t@q cp.async.cg.shared.global [%1], [%2], 16;\n\t}"
+                 ::"r"((int)on), "r"(smem_u32(dst)), "l"(src) : "memory");
+}
 __device__ __forceinline__ void cp_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void cp_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
@@ -180,8 +196,11 @@ __device__ __forceinline__ bool warp_pipeline(const Sell& A, Ring& R, int gw, in
         const int cb_a = __shfl_sync(0xffffffffu, dcur.z, src_lane);       // >= 0: 16-bit offsets from cb_a (uc_format.hpp)
         const long long eb_a = (long long)(w0 & 0x3ffffffu) << 5;
         if (info_a & kStepEnd) J = min(J, ka);
-        if (cb_a >= 0) { if (lane < (info_a & 7) * 4) cp_stream16(&R.col[sa][lane * 4], A.col16 + eb_a + lane * 8, pol_first); }
-        else if (lane < (info_a & 7) * 8) cp_stream16(&R.col[sa][lane * 4], A.col + eb_a + lane * 4, pol_first);
+        {   // one 16-byte piece per lane: nt * 4 pieces of 16-bit offsets, or nt * 8 pieces of 32-bit indices
+            const bool narrow = cb_a >= 0;
+            const char* src = narrow ? reinterpret_cast<const char*>(A.col16 + eb_a) : reinterpret_cast<const char*>(A.col + eb_a);
+            cp_stream16_if(lane < ((info_a & 7) << (narrow ? 2 : 3)), &R.col[sa][lane * 4], src + lane * 16, pol_first);
+        }
         // ---- B: values, vectors and gathers of step kb = j + kDB (its indices landed kDB commits ago)
         const long long eb = qa_e[0]; const int info_b = qa_i[0], row_b = qa_r[0], cb_b = qa_c[0];
 #pragma unroll
@@ -193,17 +212,24 @@ __device__ __forceinline__ bool warp_pipeline(const Sell& A, Ring& R, int gw, in
 #pragma unroll
             for (int k = 0; k < kChunkT / 2; ++k) {
                 const int p = k * 32 + lane;                       // 16-byte piece of the value chunk
-                if (p < nt * 16) cp_stream16(&D.val[p * 2], A.val + eb + p * 2, pol_first);
+                cp_stream16_if(p < nt * 16, &D.val[p * 2], A.val + eb + p * 2, pol_first);
             }
-            if (info_b & kStepLast) issue_vecs(D, row_b);
-            const unsigned short* c16 = reinterpret_cast<const unsigned short*>(R.col[sbA]);
-            dispatch_nt(nt, [&](auto n) {
-                int c[decltype(n)::value];
+            issue_vecs(D, row_b, (info_b & kStepLast) != 0);
+            // gathers: an index read from a stale slot entry (t >= nt) is never dereferenced
+            if (cb_b >= 0) {
+                const unsigned short* c16 = reinterpret_cast<const unsigned short*>(R.col[sbA]);
+                int c[kChunkT];
 #pragma unroll
-                for (int t = 0; t < decltype(n)::value; ++t) c[t] = cb_b >= 0 ? cb_b + (int)c16[t * 32 + lane] : R.col[sbA][t * 32 + lane];
+                for (int t = 0; t < kChunkT; ++t) c[t] = cb_b + (int)c16[t * 32 + lane];
 #pragma unroll
-                for (int t = 0; t < decltype(n)::value; ++t) cp_gather(&D.gv[t * 32 + lane], gsrc + c[t]);
-            });
+                for (int t = 0; t < kChunkT; ++t) cp_gather_if(t < nt, &D.gv[t * 32 + lane], gsrc + c[t]);
+            } else {
+                int c[kChunkT];
+#pragma unroll
+                for (int t = 0; t < kChunkT; ++t) c[t] = R.col[sbA][t * 32 + lane];
+#pragma unroll
+                for (int t = 0; t < kChunkT; ++t) cp_gather_if(t < nt, &D.gv[t * 32 + lane], gsrc + c[t]);
+            }
         }
         cp_commit();
         // ---- C: step j
@@ -275,9 +301,10 @@ __global__ void __launch_bounds__(kPrimalThreads, kCtasPerSm) k_primal(Sell KT, 
                                                        // vector v = 2k + lane/16, doubles off, off+1
     auto dep_ready = [&]() -> bool {
         grid_dependency_wait();
-        if (ld_flag(&ctl->done)) return false;
-        const int cur = ctl->cur;
-        pend = ctl->pending; eta_prev = ctl->eta_prev; tau = ctl->eta / ctl->omega;
+        const CtrlHot h = load_hot(ctl);
+        if (h.done) return false;
+        const int cur = h.cur;
+        pend = h.pending; eta_prev = h.eta_prev; tau = h.eta / h.omega;
         xcur = V.x[cur]; ycur = V.y[cur]; xnext = V.x[cur ^ 1];
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
@@ -301,10 +328,9 @@ __global__ void __launch_bounds__(kPrimalThreads, kCtasPerSm) k_primal(Sell KT, 
     } else {                                               // ---- consumer warps
         double g[1] = {0.0};
         const bool live = warp_pipeline(KT, P.w[warp], (int)blockIdx.x * kPrimalWarps + warp, lane, ycur, pol.first, dep_ready,
-            [&](auto& D, int row0) {                       // x, c, l, u (, xsum): 16 pieces of 16 bytes each
+            [&](auto& D, int row0, bool on) {              // x, c, l, u (, xsum): 16 pieces of 16 bytes each
 #pragma unroll
-                for (int k = 0; k < 3; ++k)
-                    if (vok[k]) cp_stream16(&D.vec[0][0] + voff[k], vsrc[k] + row0, pol.first);
+                for (int k = 0; k < 3; ++k) cp_stream16_if(on && vok[k], &D.vec[0][0] + voff[k], vsrc[k] + row0, pol.first);
             },
             [&](auto& D, int info, int row0) {
                 if (info & kStepFirst) g[0] = 0.0;
@@ -348,18 +374,19 @@ __global__ void __launch_bounds__(kDualThreads, kCtasPerSm) k_dual(Sell K, Vecs 
     int cur = 0, pend = 0; double eta_prev = 0.0, sig = 0.0;
     const double* ycur = nullptr; double* ynext = nullptr;
     const double* vsrc[2]; int voff[2]; bool vok[2];   // this lane's share of a slice's vector segments
-    // inputs of the step rule (A9), fetched by thread 0 of every CTA while the kernel starts and parked in shared
+    // inputs of the step rule (A9), fetched by one thread of every CTA while the kernel starts and parked in shared
     // memory: whichever CTA finishes last then runs the rule without a single cold load on the critical path of the
     // whole solve
     struct RuleIn { double eta, omega, w; long long k, acc, cap; double2 pw; uc_attempt_record* att; };
     __shared__ RuleIn rule_in;
     auto dep_ready = [&]() -> bool {
         grid_dependency_wait();
-        if (ld_flag(&ctl->done)) return false;
-        cur = ctl->cur; pend = ctl->pending; eta_prev = ctl->eta_prev; sig = ctl->eta * ctl->omega;
-        if (threadIdx.x == 0) {
+        const CtrlHot h = load_hot(ctl);
+        if (h.done) return false;
+        cur = h.cur; pend = h.pending; eta_prev = h.eta_prev; sig = h.eta * h.omega;
+        if (threadIdx.x == kDualWarps * 32) {              // the long-row warp: its dependent loads delay no slice
             RuleIn r;
-            r.eta = ctl->eta; r.omega = ctl->omega; r.w = ctl->w; r.k = ctl->k; r.acc = ctl->accepted;
+            r.eta = h.eta; r.omega = h.omega; r.w = h.w; r.k = ctl->k; r.acc = ctl->accepted;
             r.att = ctl->att; r.cap = ctl->att_cap; r.pw = ctl->powtab[r.k];     // {(k+1)^-0.6, (k+1)^-0.3} of attempt k = r.k + 1
             rule_in = r;
         }
@@ -390,11 +417,10 @@ __global__ void __launch_bounds__(kDualThreads, kCtasPerSm) k_dual(Sell K, Vecs 
     } else {                                               // ---- consumer warps
         double kx[2] = {0.0, 0.0};
         const bool live = warp_pipeline(K, P.w[warp], (int)blockIdx.x * kDualWarps + warp, lane, xg, pol.first, dep_ready,
-            [&](auto& D, int row0) {                       // y, q (, ysum): 16 pieces each; isG: 2 pieces
+            [&](auto& D, int row0, bool on) {              // y, q (, ysum): 16 pieces each; isG: 2 pieces
 #pragma unroll
-                for (int k = 0; k < 2; ++k)
-                    if (vok[k]) cp_stream16(&D.vec[0][0] + voff[k], vsrc[k] + row0, pol.first);
-                if (lane == 16 || lane == 17) cp_stream16(&D.bvec[(lane - 16) * 16], V.isG + row0 + (lane - 16) * 16, pol.first);
+                for (int k = 0; k < 2; ++k) cp_stream16_if(on && vok[k], &D.vec[0][0] + voff[k], vsrc[k] + row0, pol.first);
+                cp_stream16_if(on && (lane == 16 || lane == 17), &D.bvec[(lane & 1) * 16], V.isG + row0 + (lane & 1) * 16, pol.first);
             },
             [&](auto& D, int info, int row0) {
                 if (info & kStepFirst) { kx[0] = 0.0; kx[1] = 0.0; }
@@ -447,7 +473,7 @@ __global__ void __launch_bounds__(kDualThreads, kCtasPerSm) k_dual(Sell K, Vecs 
     if (lane != 0) return;
     ctl->ticket_b = 0;
     const double dx2 = dd_round(s3[0]), dy2 = dd_round(s3[1]), inter = fabs(dd_round(s3[2]));
-    const double r_eta = rule_in.eta, r_omega = rule_in.omega, r_w = rule_in.w;      // written by this very thread
+    const double r_eta = rule_in.eta, r_omega = rule_in.omega, r_w = rule_in.w;      // written before the block sum's barriers
     const long long r_k = rule_in.k, r_acc = rule_in.acc, r_cap = rule_in.cap;
     const double2 r_pw = rule_in.pw; uc_attempt_record* const r_att = rule_in.att;
     const double eta = r_eta, omega = r_omega;

@@ -16,6 +16,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <math.h>
+#include <stddef.h>
 #include "../../include/uc_pdhg.h"
 #include "uc_dd.cuh"
 #include "uc_format.hpp"
@@ -42,11 +43,16 @@ struct HostStatus {
 // device-resident control block: all step-size / primal-weight / restart scalars live here so that
 // the captured graph is static (SURVEY.md hard part 4)
 struct Ctrl {
-    double eta, omega, eta_prev, w, mu_prev;
-    long long k, t0, accepted, restarts, limit, nchk;
+    // ---- the first 48 bytes are what every CTA of an attempt kernel needs before it may touch the iterate: they
+    // are fetched with three 16-byte loads in ONE round trip (load_hot), on the critical path of every attempt
+    double eta, omega, eta_prev, w;
     int cur;            // which of the two x / y buffers holds the current iterate
     int pending;        // 1: the current iterate has not been added to the weighted sums yet (weight eta_prev)
-    int done, status, ret_avg, have_avg, restart_kind, cand_avg, fixed, pad0;
+    int done, status;
+    // ----
+    double mu_prev;
+    long long k, t0, accepted, restarts, limit, nchk;
+    int ret_avg, have_avg, restart_kind, cand_avg, fixed, pad0;
     KktT Tr, Tcur, Tavg;
     double eps_abs, eps_rel, beta_s, beta_n, beta_a, smoothing, norm_q, norm_c;
     unsigned int ticket_b, pad1, pad2, pad3;
@@ -57,6 +63,14 @@ struct Ctrl {
     int gen, pad4;             // generation of the solve in flight: a stop request of another generation is stale
     HostStatus* host_status;   // mapped host record
 };
+
+struct CtrlHot { double eta, omega, eta_prev, w; int cur, pending, done, status; };
+static_assert(offsetof(Ctrl, cur) == 32 && offsetof(Ctrl, status) == 44, "Ctrl hot block layout");
+__device__ __forceinline__ CtrlHot load_hot(const Ctrl* ctl) {       // L2 reads (the previous kernel wrote them)
+    const double2 a = __ldcg(reinterpret_cast<const double2*>(ctl)), b = __ldcg(reinterpret_cast<const double2*>(ctl) + 1);
+    const int4 f = __ldcg(reinterpret_cast<const int4*>(ctl) + 2);
+    return CtrlHot{a.x, a.y, b.x, b.y, f.x, f.y, f.z, f.w};
+}
 
 struct Sell {
     const long long* sp;   // slice pointers [nslices+1]
@@ -618,6 +632,11 @@ __global__ void __launch_bounds__(kBlock) k_scale_bounds(long long n, const doub
         ls[t] = (l[o] <= -1e20) ? -INFINITY : l[o] * Dc[t];
         us[t] = (u[o] >= 1e20) ? INFINITY : u[o] * Dc[t];
     }
+}
+
+__global__ void __launch_bounds__(kBlock) k_scale_cost(long long n, const double* c, const long long* perm_c, const double* Dc, double* cs) {
+    long long t = (long long)blockIdx.x * kBlock + threadIdx.x;
+    if (t < n) cs[t] = c[perm_c[t]] / Dc[t];
 }
 
 // two-stage reductions for the one-time scalars of R2 / R9: op 0 = sum of squares (double-double),

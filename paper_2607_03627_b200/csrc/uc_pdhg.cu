@@ -64,7 +64,7 @@ struct uc_lp {
     std::atomic<unsigned> state{0};
     std::atomic<int> busy{0};
     // one-time scalars
-    double eta0 = 1.0, omega0 = 1.0, norm_b = 0.0, norm_c = 0.0;
+    double eta0 = 1.0, omega0 = 1.0, norm_b = 0.0, norm_c = 0.0, norm_qs = 0.0;   // norm_qs: scaled ||q~|| (omega0 of R2)
     double precondition_seconds = 0.0, create_seconds = 0.0;
     int64_t k_slots = 0, kt_slots = 0, k_long_nnz = 0, kt_long_nnz = 0, k_narrow = 0, kt_narrow = 0;
     // step-rule factors {(k+1)^-0.6, (k+1)^-0.3}, k = 1.. (R5): a constant schedule, tabulated once
@@ -604,6 +604,7 @@ int uc_lp_create(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, cons
         lp->precondition_seconds = ms * 1e-3;
         lp->eta0 = kmax > 0.0 ? 1.0 / kmax : 1.0;
         lp->omega0 = (ncs > 1e-10 && nqs > 1e-10) ? ncs / nqs : 1.0;
+        lp->norm_qs = nqs;
         cudaFree(db); cudaFree(dc); cudaFree(dl); cudaFree(du); cudaFree(dsense); cudaFree(part); cudaFree(scal);
         lp->create_seconds = now_s() - t_create;
     } catch (const CudaFail& f) {
@@ -641,6 +642,35 @@ int uc_lp_update_bounds(uc_lp* lp, const double* l_new, const double* u_new) {
     } catch (const CudaFail& f) {
         rc = fail(UC_ERR_CUDA, std::string(f.what) + ": " + cudaGetErrorString(f.e));
     }
+    lp->busy.store(0);
+    return rc;
+}
+
+int uc_lp_update_objective(uc_lp* lp, const double* c_new) {
+    if (!lp || (lp->n > 0 && !c_new)) return fail(UC_ERR_INVALID, "NULL argument");
+    for (int64_t j = 0; j < lp->n; ++j)
+        if (!std::isfinite(c_new[j])) return fail(UC_ERR_INVALID, "c has a non-finite entry");
+    int expected = 0;
+    if (!lp->busy.compare_exchange_strong(expected, 1)) return fail(UC_ERR_BUSY, "a solve is running on this handle");
+    int rc = UC_OK;
+    double* dc = nullptr; dd* part = nullptr; double* scal = nullptr;
+    try {
+        DeviceGuard guard(lp->device);
+        cudaStream_t st = lp->own_stream;
+        const size_t bytes = sizeof(double) * (size_t)std::max<int64_t>(lp->n, 1);
+        CK(cudaMalloc((void**)&dc, bytes)); CK(cudaMalloc((void**)&part, sizeof(dd) * 1024)); CK(cudaMalloc((void**)&scal, sizeof(double)));
+        if (lp->n) CK(cudaMemcpyAsync(dc, c_new, sizeof(double) * (size_t)lp->n, cudaMemcpyHostToDevice, st));
+        lp->norm_c = std::sqrt(reduce_to_host(lp, dc, lp->n, 0, part, scal, st));            // unscaled ||c|| of R9
+        k_scale_cost<<<std::max(1, cdiv(lp->n, kBlock)), kBlock, 0, st>>>(lp->n, dc, lp->perm_c, lp->Dc, lp->cs);
+        CK(cudaGetLastError());
+        const double ncs = std::sqrt(reduce_to_host(lp, lp->cs, lp->n, 0, part, scal, st));   // R2: omega0 = ||c~|| / ||q~||
+        lp->omega0 = (ncs > 1e-10 && lp->norm_qs > 1e-10) ? ncs / lp->norm_qs : 1.0;
+    } catch (const CudaFail& f) {
+        rc = fail(UC_ERR_CUDA, std::string(f.what) + ": " + cudaGetErrorString(f.e));
+    }
+    if (dc) cudaFree(dc);
+    if (part) cudaFree(part);
+    if (scal) cudaFree(scal);
     lp->busy.store(0);
     return rc;
 }
@@ -801,6 +831,40 @@ int uc_pdhg_solve(uc_lp* lp, const uc_pdhg_params* p, double* x_out, double* y_o
 }
 int uc_pdhg_solve_device(uc_lp* lp, const uc_pdhg_params* p, double* x_out, double* y_out, uc_pdhg_result* res) {
     return solve_impl(lp, p, x_out, y_out, res, true);
+}
+
+int uc_pdhg_solve_batch(uc_lp* const* handles, int32_t count, const uc_pdhg_params* params, double* const* x_out,
+                        double* const* y_out, uc_pdhg_result* results, int32_t max_concurrent) {
+    if (count < 0 || (count > 0 && (!handles || !results))) return fail(UC_ERR_INVALID, "bad argument");
+    if (params && (params->stream || params->x0 || params->y0 || params->attempt_trace || params->check_trace))
+        return fail(UC_ERR_INVALID, "uc_pdhg_solve_batch: stream, warm start and trace fields must be NULL (they are per solve)");
+    for (int32_t i = 0; i < count; ++i) {
+        if (!handles[i]) return fail(UC_ERR_INVALID, "a handle is NULL");
+        for (int32_t j = 0; j < i; ++j) if (handles[j] == handles[i]) return fail(UC_ERR_INVALID, "the same handle appears twice");
+    }
+    const int workers = std::max(1, std::min<int>(count, max_concurrent > 0 ? max_concurrent : 16));
+    std::atomic<int32_t> next{0};
+    std::vector<int> rcs((size_t)count, UC_OK);
+    std::vector<std::string> errs((size_t)count);
+    auto work = [&]() {
+        for (;;) {
+            const int32_t i = next.fetch_add(1);
+            if (i >= count) return;
+            rcs[(size_t)i] = solve_impl(handles[i], params, x_out ? x_out[i] : nullptr, y_out ? y_out[i] : nullptr, &results[i], false);
+            if (rcs[(size_t)i] != UC_OK) errs[(size_t)i] = g_err;       // thread-local text of the worker
+        }
+    };
+    try {
+        std::vector<std::thread> th;
+        for (int w = 1; w < workers; ++w) th.emplace_back(work);
+        work();
+        for (auto& t : th) t.join();
+    } catch (const std::exception& e) {
+        return fail(UC_ERR_NOMEM, std::string("uc_pdhg_solve_batch: ") + e.what());
+    }
+    for (int32_t i = 0; i < count; ++i)
+        if (rcs[(size_t)i] != UC_OK) return fail(rcs[(size_t)i], "solve " + std::to_string(i) + ": " + errs[(size_t)i]);
+    return UC_OK;
 }
 
 int uc_pdhg_time_kernels(uc_lp* lp, void* stream, int32_t attempts, double* primal_ms, double* dual_ms) {

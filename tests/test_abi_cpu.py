@@ -75,6 +75,11 @@ def test_invalid_arguments_are_rejected_before_touching_a_device():
     assert lib.uc_pdhg_cancel(None) == -1
     assert lib.uc_pdhg_solve(None, None, None, None, None) == -1
     lib.uc_lp_destroy(None)                                   # NULL is fine
+    assert lib.uc_lp_update_objective(None, None) == -1 and lib.uc_lp_update_bounds(None, None, None) == -1
+    res = (binding.Result * 2)()
+    two_null = (C.c_void_p * 2)(None, None)
+    assert lib.uc_pdhg_solve_batch(C.cast(two_null, C.c_void_p), 2, None, None, None, C.cast(res, C.c_void_p), 0) == -1
+    assert lib.uc_pdhg_solve_batch(None, 0, None, None, None, None, 0) == 0      # an empty batch is not an error
 
 
 def test_no_cpu_fallback_without_a_device():

@@ -127,3 +127,26 @@ def test_different_handles_solve_concurrently_on_their_own_streams(lp1):
     finally:
         for h in handles:
             h.close()
+
+
+def test_solve_batch_results_are_those_of_solo_solves(lp1):
+    """uc_pdhg_solve_batch (the paper's 45 scenarios, P:l.101): different LPs solved concurrently
+    inside one call, fewer workers than handles; every result is bit-identical to the solve run alone."""
+    lps = [uc_config(0), lp1, uc_config("tuned_presolve"), uc_config(0), lp1, uc_config("tuned_presolve"), uc_config(0)]
+    handles = [P.UcLp(lp) for lp in lps]
+    try:
+        solo = [h.solve(fixed_iterations=320) for h in handles[:3]]
+        out = P.solve_batch(handles, max_concurrent=3, fixed_iterations=320)
+        assert len(out) == len(handles)
+        for i, s in enumerate(out):
+            assert s.status == P.ITERATION_LIMIT and s.iterations == 320
+            assert np.array_equal(s.x, solo[i % 3].x) and np.array_equal(s.y, solo[i % 3].y)
+        conv = P.solve_batch(handles[:3])                         # default stopping rule
+        for s, h in zip(conv, handles[:3]):
+            alone = h.solve()
+            assert s.status == P.OPTIMAL and s.iterations == alone.iterations and s.primal_obj == alone.primal_obj
+        with pytest.raises(P.UcError):
+            P.solve_batch([handles[0], handles[0]])               # the same handle twice
+    finally:
+        for h in handles:
+            h.close()

@@ -373,6 +373,57 @@ def test_fixed_commitment_resolve_with_update_bounds():
     assert again.iterations == relaxed.iterations and again.primal_obj == relaxed.primal_obj
 
 
+def test_warm_started_fixed_commitment_resolve_matches_oracle():
+    """SURVEY.md 8(f) NEXT-2 (P:l.60 "relaxed", l.62 re-solves): fix the commitment with uc_lp_update_bounds and re-solve
+    FROM THE PREVIOUS (x, y); the oracle does the same on the fixed LP with the same warm start."""
+    lp = get_lp("uc0")
+    G, T, V, oU = lp.meta["G"], lp.meta["T"], lp.meta["V"], lp.meta["offsets"]["u"]
+    with P.UcLp(lp) as h:
+        relaxed = h.solve()
+        pattern = (relaxed.x.reshape(T, V)[:, oU:oU + G].T > 0.5).astype(float)
+        fixed = fix_commitment(lp, pattern)
+        h.update_bounds(fixed.l, fixed.u)
+        cold = h.solve(trace_checks=4096)
+        warm = h.solve(x0=relaxed.x, y0=relaxed.y, trace_checks=4096)
+        warm200 = h.solve(x0=relaxed.x, y0=relaxed.y, fixed_iterations=200)
+    so = oracle.solve(fixed, x0=relaxed.x, y0=relaxed.y)
+    so200 = oracle.solve(fixed, x0=relaxed.x, y0=relaxed.y, fixed_iterations=200)
+    assert warm.status == P.OPTIMAL == so.status and warm.iterations == so.iterations and warm.restarts == so.restarts
+    assert abs(warm.primal_obj - so.primal_obj) <= TOL_OBJ * (1 + abs(so.primal_obj))
+    np.testing.assert_array_equal(warm.checks["restart_kind"], so.checks["restart_kind"])
+    assert rel_l2(warm200.x, so200.x) <= TOL_ITER and rel_l2(warm200.y, so200.y) <= TOL_ITER
+    assert abs(warm.primal_obj - cold.primal_obj) <= 2e-4 * (1 + abs(cold.primal_obj))      # same LP, both at 1e-4
+    assert warm.iterations <= cold.iterations
+
+
+def test_update_objective_equals_a_fresh_handle_and_the_oracle():
+    """uc_lp_update_objective: the handle behaves like one created with the new c (the scalings do not depend on c)."""
+    from workloads.lp import LP
+    lp = get_lp("uc0")
+    rng = np.random.default_rng(17)
+    c2 = lp.c * rng.uniform(0.5, 1.5, lp.n)
+    lp2 = LP(m=lp.m, n=lp.n, row_ptr=lp.row_ptr, col_idx=lp.col_idx, val=lp.val, sense=lp.sense, b=lp.b, c=c2, l=lp.l, u=lp.u)
+    so = oracle.solve(lp2, fixed_iterations=200, trace_attempts=200)
+    with P.UcLp(lp) as h:
+        first = h.solve(fixed_iterations=200)
+        h.update_objective(c2)
+        sg = h.solve(fixed_iterations=200, trace_attempts=200)
+        conv = h.solve()
+        h.update_objective(lp.c)
+        back = h.solve(fixed_iterations=200)
+        with pytest.raises(P.UcError):
+            h.update_objective(np.full(lp.n, np.nan))
+    with P.UcLp(lp2) as h2:
+        fresh = h2.solve(fixed_iterations=200)
+    np.testing.assert_array_equal(sg.x, fresh.x); np.testing.assert_array_equal(sg.y, fresh.y)
+    np.testing.assert_array_equal(back.x, first.x); np.testing.assert_array_equal(back.y, first.y)
+    np.testing.assert_array_equal(sg.attempts["accepted"], so.attempts["accepted"])
+    assert rel_l2(sg.x, so.x) <= TOL_ITER and rel_l2(sg.y, so.y) <= TOL_ITER
+    oc = oracle.solve(lp2)
+    assert conv.status == P.OPTIMAL and conv.iterations == oc.iterations
+    assert abs(conv.primal_obj - oc.primal_obj) <= TOL_OBJ * (1 + abs(oc.primal_obj))
+
+
 def test_solves_are_reproducible_bit_for_bit():
     lp = get_lp("uc1")
     with P.UcLp(lp) as h:

@@ -79,3 +79,12 @@ def test_random_lp_recipe():
     for i in range(0, 200):                                                             # sorted, no duplicates
         cols = lp.col_idx[lp.row_ptr[i]:lp.row_ptr[i + 1]]
         assert np.all(np.diff(cols) > 0)
+
+
+def test_tuned_presolve_shape_workload():
+    """PAPER.md Table VII (l.241-246): the tuned presolve hands PDHG a 38,238 x 44,822 LP; the named workload has that shape."""
+    from workloads import uc_config
+    lp = uc_config("tuned_presolve")
+    lp.validate()
+    assert abs(lp.m - 38238) <= 0.01 * 38238 and abs(lp.n - 44822) <= 0.01 * 44822
+    assert lp.name == "uc_tuned_presolve"

@@ -30,16 +30,19 @@ UC_CONFIGS = {
     1: dict(B=500, L=700, G=90, T=48, dt_hours=1.0, min_updown=False, seed=1),
     2: dict(B=2000, L=3200, G=300, T=48, dt_hours=1.0, min_updown=True, seed=2),
     3: dict(B=6049, L=8000, G=800, T=96, dt_hours=0.25, min_updown=True, seed=3),
+    # not a BASELINE.json config: the SHAPE of the LP the paper's tuned presolve hands to PDHG, 38,238 x 44,822
+    # (Table VII l.241-246; Table VI l.221-226: the GPU loses all 45 races there) -> 38,168 x 44,928 here
+    "tuned_presolve": dict(B=138, L=200, G=92, T=48, dt_hours=1.0, min_updown=False, seed=5),
 }
 
 SHED_PENALTY = 1e4
 RESERVE_FRACTION = 0.05
 
 
-def uc_config(i: int) -> LP:
+def uc_config(i) -> LP:
     cfg = UC_CONFIGS[i]
     lp = uc_lp(**cfg)
-    lp.name = f"uc_config{i}"
+    lp.name = f"uc_config{i}" if isinstance(i, int) else f"uc_{i}"
     return lp
 
 
