@@ -182,6 +182,16 @@ int uc_pdhg_cancel(uc_lp* lp);
    NULL.  The handle's iterate state is overwritten. */
 int uc_pdhg_time_kernels(uc_lp* lp, void* stream, int32_t attempts, double* primal_ms, double* dual_ms);
 
+/* Measurement hook, only in a library built with -DUC_TIMELINE (otherwise UC_ERR_INVALID): run `attempts` attempts from
+   the initial point as plain stream launches (programmatic dependent launch, no events in between) and return the
+   %globaltimer marks (ns) that every warp of the two kernels of the LAST attempt recorded:
+   out[((cta * 32 + warp) * 8) + i], i = 0 kernel entry, 1 grid dependency resolved, 2 own steps done, 3 block sum done
+   (for the warp that ran the step rule: attempt decided), 4 ticket taken, 5 partials of all CTAs loaded, 6 final sums
+   done (4-6: warp 0 of the dual kernel only); the dual kernel's block starts at out + grid_primal * 32 * 8.
+   out: HOST buffer of `cap` entries, cap >= (grid_primal + grid_dual) * 256; unused entries stay 0.
+   and profiles/ use it for the timeline of an attempt. */
+int uc_pdhg_timeline(uc_lp* lp, void* stream, int32_t attempts, uint64_t* out, int64_t cap, int32_t* grid_primal, int32_t* grid_dual);
+
 /* ------------------------------------------------------------------------------- introspection */
 typedef struct {
     int64_t m, n, nnz;
@@ -212,12 +222,13 @@ int uc_lp_get_scaled_values(uc_lp* lp, int32_t from_transpose, double* val_out);
 int uc_lp_spmv(uc_lp* lp, int32_t transpose, const double* v, double* out);
 
 /* Host-only self-check of ingest step A1 (no GPU needed): builds the row / column permutations, the explicit
-   transpose, both SELL-32 layouts and both attempt schedules (for `sched_warps` consumer warps) exactly as
-   uc_lp_create does, and verifies them entry by entry against the caller's CSR: stored entries are the caller's, in
-   the caller's order (K' rows in ascending caller row index), padding is (0, 0.0), every slice is scheduled exactly
-   once as consecutive chunks.  Returns UC_OK, or UC_ERR_INVALID with the violated property in uc_last_error(). */
+   transpose, both SELL-32 layouts and both attempt schedules (for `sched_ctas` CTAs of `warps_per_cta` consumer warps)
+   exactly as uc_lp_create does, and verifies them entry by entry against the caller's CSR: stored entries are the
+   caller's, in the caller's order (K' rows in ascending caller row index), padding is (0, 0.0), every slice is scheduled
+   exactly once as consecutive chunks, and the slices of a CTA form one contiguous range (CTA c's before CTA c+1's).
+   Returns UC_OK, or UC_ERR_INVALID with the violated property in uc_last_error(). */
 int uc_host_layout_selftest(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, const int32_t* col_idx, const double* val,
-                            int32_t sell_window, int32_t long_row_threshold, int32_t sched_warps);
+                            int32_t sell_window, int32_t long_row_threshold, int32_t sched_ctas, int32_t warps_per_cta);
 
 /* Host evaluation of the double-double log / exp that the primal-weight update (R11) runs on the
    device (same source, csrc/uc_dd.cuh).  Test hooks: no GPU needed. */

@@ -60,7 +60,7 @@ CHECK_DTYPE = np.dtype([("k", "i8"), ("restart_kind", "i4"), ("candidate", "i4")
                         ("mu_c", "f8"), ("mu_r", "f8"), ("relkkt_cur", "f8"), ("relkkt_avg", "f8")])
 
 EXPORTS = ["uc_lp_default_options", "uc_lp_create", "uc_lp_update_bounds", "uc_lp_update_objective", "uc_lp_destroy",
-           "uc_pdhg_default_params", "uc_pdhg_solve", "uc_pdhg_solve_device", "uc_pdhg_solve_batch", "uc_pdhg_cancel", "uc_pdhg_time_kernels",
+           "uc_pdhg_default_params", "uc_pdhg_solve", "uc_pdhg_solve_device", "uc_pdhg_solve_batch", "uc_pdhg_cancel", "uc_pdhg_time_kernels", "uc_pdhg_timeline",
            "uc_lp_get_info", "uc_lp_get_scaling", "uc_lp_get_scaled_values", "uc_lp_spmv", "uc_last_error",
            "uc_host_log_rounded", "uc_host_exp_rounded", "uc_host_layout_selftest"]
 
@@ -98,8 +98,9 @@ def load_library(build_if_missing: bool = True):
     lib.uc_pdhg_solve_device.argtypes = [C.c_void_p] * 5
     lib.uc_pdhg_solve_batch.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32]
     lib.uc_pdhg_time_kernels.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
+    lib.uc_pdhg_timeline.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
     lib.uc_host_layout_selftest.argtypes = [C.c_int64, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p,
-                                            C.c_int32, C.c_int32, C.c_int32]
+                                            C.c_int32, C.c_int32, C.c_int32, C.c_int32]
     lib.uc_lp_get_info.argtypes = [C.c_void_p] * 2
     lib.uc_lp_get_scaling.argtypes = [C.c_void_p] * 3
     lib.uc_lp_get_scaled_values.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
@@ -113,13 +114,13 @@ def _check(rc):
         raise UcError(rc, load_library().uc_last_error().decode())
 
 
-def host_layout_selftest(lp, sell_window=4096, long_row_threshold=32, sched_warps=148 * 15) -> None:
+def host_layout_selftest(lp, sell_window=4096, long_row_threshold=32, sched_ctas=148, warps_per_cta=15) -> None:
     """uc_host_layout_selftest on a workloads.LP; raises UcError with the violated property."""
     lib = load_library()
     rp = np.ascontiguousarray(lp.row_ptr, dtype=np.int64); ci = np.ascontiguousarray(lp.col_idx, dtype=np.int32)
     va = np.ascontiguousarray(lp.val, dtype=np.float64)
     _check(lib.uc_host_layout_selftest(int(lp.m), int(lp.n), int(lp.nnz), C.c_void_p(rp.ctypes.data), C.c_void_p(ci.ctypes.data),
-                                       C.c_void_p(va.ctypes.data), int(sell_window), int(long_row_threshold), int(sched_warps)))
+                                       C.c_void_p(va.ctypes.data), int(sell_window), int(long_row_threshold), int(sched_ctas), int(warps_per_cta)))
 
 
 def default_options(**kw) -> Options:
@@ -248,6 +249,20 @@ class UcLp:
         return a.value, b.value
 
     time_kernels = uc_pdhg_time_kernels
+
+    def uc_pdhg_timeline(self, attempts=16, stream=None):
+        """(primal, dual) arrays [grid, 32 warps, 8 marks] of %globaltimer ns for the last of `attempts` attempts
+        (a -DUC_TIMELINE build only)."""
+        cap = 2 * 1024 * 256
+        out = np.zeros(cap, dtype=np.uint64)
+        gp, gd = C.c_int32(0), C.c_int32(0)
+        _check(self.lib.uc_pdhg_timeline(self._h, C.c_void_p(int(stream)) if stream else None, int(attempts),
+                                         out.ctypes.data_as(C.c_void_p), C.c_int64(cap), C.byref(gp), C.byref(gd)))
+        a = out[: gp.value * 256].reshape(gp.value, 32, 8)
+        b = out[gp.value * 256: (gp.value + gd.value) * 256].reshape(gd.value, 32, 8)
+        return a, b
+
+    timeline = uc_pdhg_timeline
 
     def info(self) -> Info:
         i = Info()

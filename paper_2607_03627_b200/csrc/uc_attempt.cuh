@@ -89,21 +89,35 @@ __device__ __forceinline__ void cp_gather(double* dst, const double* src) {
 __device__ __forceinline__ void cp_gather(double2* dst, const double2* src) {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"(src) : "memory");   // L1 bypass: measured faster
 }
-// Predicated forms: `on` becomes a predicate on the copy itself.  The conditions below are warp-uniform functions of
-// the step descriptor, but the compiler cannot know that (the descriptor comes out of a shuffle), so an `if` around a
-// copy costs a BSSY / BRA / BSYNC triple; ncu showed control flow at 21 % of the instructions of the loop, which is
-// bound by instruction issue latency at 4 warps per scheduler (profiles/r02a).
-__device__ __forceinline__ void cp_stream16_if(bool on, void* dst, const void* src, uint64_t pol) {
-    asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.s32 q, %0, 0;\n\t@q cp.async.cg.shared.global.L2::cache_hint [%1], [%2], 16, %3;\n\t}"
-                 ::"r"((int)on), "r"(smem_u32(dst)), "l"(src), "l"(pol) : "memory");
+// Predicated forms: the comparison `a < b` becomes a predicate on the copy itself.  The conditions below are warp-uniform
+// functions of the step descriptor, but the compiler cannot know that (the descriptor comes out of a shuffle), so an
+// `if` around a copy costs a BSSY / BRA / BSYNC triple; the loop is bound by instruction issue latency at 4 warps per
+// scheduler (profiles/r02a), so every instruction on a warp's dependent chain counts.
+__device__ __forceinline__ void cp_stream16_lt(int a, int b, void* dst, const void* src, uint64_t pol) {
+    asm volatile("{\n\t.reg .pred q;\n\tsetp.lt.s32 q, %0, %1;\n\t@q cp.async.cg.shared.global.L2::cache_hint [%2], [%3], 16, %4;\n\t}"
+                 ::"r"(a), "r"(b), "r"(smem_u32(dst)), "l"(src), "l"(pol) : "memory");
 }
-__device__ __forceinline__ void cp_gather_if(bool on, double* dst, const double* src) {
-    asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.s32 q, %0, 0;\n\t@q cp.async.ca.shared.global [%1], [%2], 8;\n\t}"
-                 ::"r"((int)on), "r"(smem_u32(dst)), "l"(src) : "memory");
+__device__ __forceinline__ void cp_gather_lt(int a, int b, double* dst, const double* src) {
+    asm volatile("{\n\t.reg .pred q;\n\tsetp.lt.s32 q, %0, %1;\n\t@q cp.async.ca.shared.global [%2], [%3], 8;\n\t}"
+                 ::"r"(a), "r"(b), "r"(smem_u32(dst)), "l"(src) : "memory");
 }
-__device__ __forceinline__ void cp_gather_if(bool on, double2* dst, const double2* src) {
-    asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.s32 q, %0, 0;\n\t@q cp.async.cg.shared.global [%1], [%2], 16;\n\t}"
-                 ::"r"((int)on), "r"(smem_u32(dst)), "l"(src) : "memory");
+#ifndef UC_DUAL_GATHER
+#define UC_DUAL_GATHER "ca"
+#endif
+__device__ __forceinline__ void cp_gather_lt(int a, int b, double2* dst, const double2* src) {
+    asm volatile("{\n\t.reg .pred q;\n\tsetp.lt.s32 q, %0, %1;\n\t@q cp.async." UC_DUAL_GATHER ".shared.global [%2], [%3], 16;\n\t}"
+                 ::"r"(a), "r"(b), "r"(smem_u32(dst)), "l"(src) : "memory");
+}
+// column index of a stored entry, straight into a register (streamed once: no L1 allocation), only if a < b; `v` keeps
+// its old value otherwise (never used: the gather it would feed carries the same predicate)
+__device__ __forceinline__ void ld_index_lt(int a, int b, int& v, const unsigned short* p) {
+    // a 16-bit load may name a 32-bit destination (zero-extended): one predicated LDG, nothing that depends on it here
+    asm("{\n\t.reg .pred q;\n\tsetp.lt.s32 q, %1, %2;\n\t@q ld.global.nc.L1::no_allocate.u16 %0, [%3];\n\t}"
+        : "+r"(v) : "r"(a), "r"(b), "l"(p));
+}
+__device__ __forceinline__ void ld_index_lt(int a, int b, int& v, const int* p) {
+    asm("{\n\t.reg .pred q;\n\tsetp.lt.s32 q, %1, %2;\n\t@q ld.global.nc.L1::no_allocate.s32 %0, [%3];\n\t}"
+        : "+r"(v) : "r"(a), "r"(b), "l"(p));
 }
 __device__ __forceinline__ void cp_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
@@ -118,18 +132,23 @@ struct Policies { uint64_t first, last; };
 
 // ------------------------------------------------------------------------------------------ per-warp rings
 // GT: what one entry gathers -- double (y) or double2 ({xbar, dx}).  Everything in here is private to ONE warp.
+// A slot is a multiple of 128 bytes: an asynchronous copy whose shared-memory destination is not aligned like its global
+// source (16 bytes off, as the second slot of the primal ring was) is split at the shared-memory sector boundaries and
+// fetches every 32-byte global sector TWICE (profiles/r02b: 2.2 M of 6.6 M L2 sectors of the streamed data per launch).
 template <int NVEC, bool BYTEVEC, class GT>
-struct DataSlot {
+struct alignas(128) DataSlot {
     double val[kChunkE];
     GT gv[kChunkE];              // gv[e] = gathered vector entry for stored entry e
     double vec[NVEC][32];        // 32-row segments of the per-row vectors (last step of a slice only)
     unsigned char bvec[BYTEVEC ? 32 : 16];
 };
+// DB = how many steps the data copies run ahead of the compute: 1 (two slots) or 3 (four slots); the slot of step s
+// is s & (kSlots - 1), a compile-time constant in the loop below (unrolled by four)
 template <int NVEC, bool BYTEVEC, class GT, int DB>
 struct WarpRing {
-    static constexpr int kDB = DB, kDA = 2 * DB + 1, kRingA = DB + 2, kRingB = DB + 1;
-    int col[kRingA][kChunkE];
-    DataSlot<NVEC, BYTEVEC, GT> data[kRingB];
+    static_assert(DB == 1 || DB == 3, "data ring: 2 or 4 slots");
+    static constexpr int kDB = DB, kSlots = DB + 1;
+    DataSlot<NVEC, BYTEVEC, GT> data[kSlots];
 };
 template <int NVEC, bool BYTEVEC, class GT, int WARPS, int DB>
 struct SmemT {
@@ -158,92 +177,128 @@ __device__ __forceinline__ void dispatch_nt(int nt, F f) {
 }
 
 // ------------------------------------------------------------------------------------------ the pipeline
-// Runs the steps of consumer warp `gw` (of A.sched_warps) through the A / B / C pipeline described at the top.
-//   issue_vecs(slot, row0)    issues the cp.async copies of the 32-row vector segments of a slice
-//   compute(slot, info, row0) consumes one step from shared memory
-// The schedule is read 32 steps at a time (lane l holds step 32 b + l of the warp; the next batch is loaded
-// one batch ahead) and a step's descriptor travels from A to B to C through two small register queues, so
-// only the A cursor ever touches it.
-// dep_ready() is called once, just before the first B stage: everything before it (schedule loads, the first
-// index copies) touches only data that no kernel writes, so it overlaps the tail of the previous kernel
-// (programmatic dependent launch); it returns false if the solve is already over.
+// Runs the steps of consumer warp `gw` (of A.sched_warps) through a three-stage software pipeline.  In the iteration
+// that computes step j the warp also issues
+//     A(j + DB + 2): plain loads of the step's column indices into REGISTERS (coalesced, 2 or 4 bytes per lane and
+//                    entry; they are consumed two iterations later, so their latency is off the dependent chain)
+//     B(j + DB):     cp.async of the step's matrix values, of the 32-row segments of the per-row vectors (last step
+//                    of a slice only) and one 8/16-byte cp.async per stored entry, gv[e] <- src[col[e]]  -> data ring
+//     C(j):          everything read from shared memory: row sums left to right, update, coalesced stores.
+//   issue_vecs(slot, row0, last01)  issues the cp.async copies of the 32-row vector segments of a slice
+//   compute(slot, info, row0)       consumes one step from shared memory
+// The loop is unrolled by four with every ring slot and queue position a compile-time constant: the kernel is bound by
+// instruction issue latency (4 warps per scheduler, each a long dependent chain), so the bookkeeping of a step --
+// queue rotation, slot wrap-around, address arithmetic -- was as expensive as its arithmetic before (profiles/r02a:
+// 252 SASS instructions per step, 19 of them register moves at the loop head).
+// The schedule is read 32 steps at a time (lane l holds step 32 b + l of the warp; the next batch is loaded one batch
+// ahead) and handed from stage to stage in registers.
+// dep_ready() is called once, just before the first B stage: everything before it (schedule loads, the first index
+// loads) touches only data that no kernel writes, so it overlaps the tail of the previous kernel (programmatic
+// dependent launch); it returns false if the solve is already over.
 template <class Ring, class GT, class FD, class FV, class FC>
 __device__ __forceinline__ bool warp_pipeline(const Sell& A, Ring& R, int gw, int lane, const GT* const& gsrc,
                                               uint64_t pol_first, FD dep_ready, FV issue_vecs, FC compute) {
-    constexpr int kDB = Ring::kDB, kDA = Ring::kDA, kRingA = Ring::kRingA, kRingB = Ring::kRingB;
+    constexpr int DB = Ring::kDB, NS = Ring::kSlots, DA = DB + 2;
     int J = A.steps_per_warp;                                      // shrinks to this warp's own count at its end marker
     const long long GW = A.sched_warps;
     auto load_desc = [&](int k) -> int4 {
         return k < J ? __ldg(reinterpret_cast<const int4*>(A.steps + (long long)k * GW + gw)) : make_int4(0, 0, -1, 0);
     };
     int4 dcur = load_desc(lane), dnxt = load_desc(32 + lane);
-    long long qa_e[kDA - kDB]; int qa_i[kDA - kDB], qa_r[kDA - kDB], qa_c[kDA - kDB];     // A -> B
-    int qb_i[kDB], qb_r[kDB];                                            // B -> C
+    // A -> B, position = step & 3: descriptor fields and the column indices of the lane's entries
+    int q_info[4] = {0, 0, 0, 0}, q_row[4] = {0, 0, 0, 0}, q_cb[4] = {-1, -1, -1, -1}, q_idx[4][kChunkT];
+    unsigned q_eb[4] = {0u, 0u, 0u, 0u};
 #pragma unroll
-    for (int q = 0; q < kDA - kDB; ++q) { qa_e[q] = 0; qa_i[q] = 0; qa_r[q] = 0; qa_c[q] = -1; }
+    for (int q = 0; q < 4; ++q)
 #pragma unroll
-    for (int q = 0; q < kDB; ++q) { qb_i[q] = 0; qb_r[q] = 0; }
-    // ring slots of steps ka (index ring), kb (index ring: kb = ka - (kRingA - 1)), kb (data ring: kb = -kRingB at the start), j
-    int sa = 0, sbA = 1 % kRingA, sb = 0, sc = 0;
-    for (int j = -kDA; j < J; ++j) {
-        if (j == -kDB && !dep_ready()) { cp_wait<0>(); return false; }
-        // ---- A: column indices of step ka = j + kDA
-        const int ka = j + kDA;
-        if (ka >= 32 && (ka & 31) == 0) { dcur = dnxt; dnxt = load_desc(ka + 32 + lane); }
-        const int src_lane = ka & 31;
-        const unsigned w0 = (unsigned)__shfl_sync(0xffffffffu, dcur.x, src_lane);
-        const int row_a = __shfl_sync(0xffffffffu, dcur.y, src_lane), info_a = (int)(w0 >> 26);
-        const int cb_a = __shfl_sync(0xffffffffu, dcur.z, src_lane);       // >= 0: 16-bit offsets from cb_a (uc_format.hpp)
-        const long long eb_a = (long long)(w0 & 0x3ffffffu) << 5;
-        if (info_a & kStepEnd) J = min(J, ka);
-        {   // one 16-byte piece per lane: nt * 4 pieces of 16-bit offsets, or nt * 8 pieces of 32-bit indices
-            const bool narrow = cb_a >= 0;
-            const char* src = narrow ? reinterpret_cast<const char*>(A.col16 + eb_a) : reinterpret_cast<const char*>(A.col + eb_a);
-            cp_stream16_if(lane < ((info_a & 7) << (narrow ? 2 : 3)), &R.col[sa][lane * 4], src + lane * 16, pol_first);
+        for (int t = 0; t < kChunkT; ++t) q_idx[q][t] = 0;
+    // B -> C, position = data slot
+    int c_info[NS], c_row[NS];
+#pragma unroll
+    for (int q = 0; q < NS; ++q) { c_info[q] = 0; c_row[q] = 0; }
+
+    // one iteration; P = j & 3 at compile time; PRO: prologue (no compute, stages of negative steps skipped)
+    auto body = [&](auto Pc, auto PROc, const int j) {
+        constexpr int P = decltype(Pc)::value;
+        constexpr bool PRO = decltype(PROc)::value != 0;
+        // ---- A: column indices of step sa = j + DA
+        const int sa = j + DA;
+        if (!PRO || sa >= 0) {
+            constexpr int qa = (P + DA) & 3;
+            if constexpr (qa == 0 && !PRO) {                      // sa is a multiple of 4 here: a batch may begin
+                if ((sa & 31) == 0) { dcur = dnxt; dnxt = load_desc(sa + 32 + lane); }
+            }
+            const int src_lane = sa & 31;
+            const unsigned w0 = (unsigned)__shfl_sync(0xffffffffu, dcur.x, src_lane);
+            const int row_a = __shfl_sync(0xffffffffu, dcur.y, src_lane);
+            const int cb_a = __shfl_sync(0xffffffffu, dcur.z, src_lane);   // >= 0: 16-bit offsets from cb_a (uc_format.hpp)
+            const int info_a = (int)(w0 >> 26), nt = info_a & 7;
+            const unsigned eb32 = w0 & 0x3ffffffu;                          // first stored entry of the step / 32
+            if (info_a & kStepEnd) J = min(J, sa);
+            q_info[qa] = info_a; q_row[qa] = row_a; q_cb[qa] = cb_a < 0 ? 0 : cb_a; q_eb[qa] = eb32;
+            const long long e0 = ((long long)eb32 << 5) + lane;
+            if (cb_a >= 0) {
+                const unsigned short* p = A.col16 + e0;
+#pragma unroll
+                for (int t = 0; t < kChunkT; ++t) ld_index_lt(t, nt, q_idx[qa][t], p + 32 * t);
+            } else {
+                const int* p = A.col + e0;
+#pragma unroll
+                for (int t = 0; t < kChunkT; ++t) ld_index_lt(t, nt, q_idx[qa][t], p + 32 * t);
+            }
         }
-        // ---- B: values, vectors and gathers of step kb = j + kDB (its indices landed kDB commits ago)
-        const long long eb = qa_e[0]; const int info_b = qa_i[0], row_b = qa_r[0], cb_b = qa_c[0];
-#pragma unroll
-        for (int q = 0; q + 1 < kDA - kDB; ++q) { qa_e[q] = qa_e[q + 1]; qa_i[q] = qa_i[q + 1]; qa_r[q] = qa_r[q + 1]; qa_c[q] = qa_c[q + 1]; }
-        qa_e[kDA - kDB - 1] = eb_a; qa_i[kDA - kDB - 1] = info_a; qa_r[kDA - kDB - 1] = row_a; qa_c[kDA - kDB - 1] = cb_a;
-        {
-            const int nt = info_b & 7;
-            auto& D = R.data[sb];
+        // ---- B: values, vectors and gathers of step sb = j + DB
+        const int sb = j + DB;
+        if (!PRO || sb >= 0) {
+            constexpr int qb = (P + DB) & 3, db = (P + DB) & (NS - 1);
+            const int info_b = q_info[qb], row_b = q_row[qb], nt = info_b & 7;
+            auto& D = R.data[db];
+            const double* vsrc = A.val + ((long long)q_eb[qb] << 5);
 #pragma unroll
             for (int k = 0; k < kChunkT / 2; ++k) {
                 const int p = k * 32 + lane;                       // 16-byte piece of the value chunk
-                cp_stream16_if(p < nt * 16, &D.val[p * 2], A.val + eb + p * 2, pol_first);
+                cp_stream16_lt(p, nt * 16, &D.val[p * 2], vsrc + p * 2, pol_first);
             }
-            issue_vecs(D, row_b, (info_b & kStepLast) != 0);
-            // gathers: an index read from a stale slot entry (t >= nt) is never dereferenced
-            if (cb_b >= 0) {
-                const unsigned short* c16 = reinterpret_cast<const unsigned short*>(R.col[sbA]);
-                int c[kChunkT];
+            issue_vecs(D, row_b, (info_b >> 4) & 1);               // kStepLast
+            const GT* gs = gsrc + q_cb[qb];
 #pragma unroll
-                for (int t = 0; t < kChunkT; ++t) c[t] = cb_b + (int)c16[t * 32 + lane];
-#pragma unroll
-                for (int t = 0; t < kChunkT; ++t) cp_gather_if(t < nt, &D.gv[t * 32 + lane], gsrc + c[t]);
-            } else {
-                int c[kChunkT];
-#pragma unroll
-                for (int t = 0; t < kChunkT; ++t) c[t] = R.col[sbA][t * 32 + lane];
-#pragma unroll
-                for (int t = 0; t < kChunkT; ++t) cp_gather_if(t < nt, &D.gv[t * 32 + lane], gsrc + c[t]);
-            }
+#ifdef UC_EXP_COALESCED
+            for (int t = 0; t < kChunkT; ++t) cp_gather_lt(t, nt, &D.gv[t * 32 + lane], gsrc + (row_b / 2 + 32 * t + lane));
+#else
+            for (int t = 0; t < kChunkT; ++t) cp_gather_lt(t, nt, &D.gv[t * 32 + lane], gs + q_idx[qb][t]);
+#endif
+            c_info[db] = info_b; c_row[db] = row_b;
+            cp_commit();
         }
-        cp_commit();
         // ---- C: step j
-        const int info_c = qb_i[0], row_c = qb_r[0];
+        if constexpr (!PRO) {
+            constexpr int dc = P & (NS - 1);
+            cp_wait<DB>();
+            __syncwarp();                                          // the copies of every lane are visible to the warp
+            if (c_info[dc]) compute(R.data[dc], c_info[dc], c_row[dc]);
+            __syncwarp();                                          // the slot is rewritten by the next iteration's copies
+        }
+    };
+    static_assert(kStepLast == 16, "issue_vecs takes bit 4 of the step info");
+    constexpr int kPro = (DA + 3) & ~3;                            // prologue iterations (a multiple of four)
+    bool live = true;
 #pragma unroll
-        for (int q = 0; q + 1 < kDB; ++q) { qb_i[q] = qb_i[q + 1]; qb_r[q] = qb_r[q + 1]; }
-        qb_i[kDB - 1] = info_b; qb_r[kDB - 1] = row_b;
-        cp_wait<kDB>();
-        __syncwarp();                                              // the copies of every lane are visible to the warp
-        if (info_c) compute(R.data[sc], info_c, row_c);
-        __syncwarp();                                              // slots are rewritten by the next iteration's copies
-        sa = (sa + 1 == kRingA) ? 0 : sa + 1; sbA = (sbA + 1 == kRingA) ? 0 : sbA + 1;
-        sb = (sb + 1 == kRingB) ? 0 : sb + 1;
-        if (j >= 0) sc = (sc + 1 == kRingB) ? 0 : sc + 1;
+    for (int i = 0; i < kPro; ++i) {
+        const int j = i - kPro;
+        if (j == -DB) { live = dep_ready(); if (!live) break; }
+        switch (i & 3) {
+            case 0: body(IntC<0>{}, IntC<1>{}, j); break;
+            case 1: body(IntC<1>{}, IntC<1>{}, j); break;
+            case 2: body(IntC<2>{}, IntC<1>{}, j); break;
+            default: body(IntC<3>{}, IntC<1>{}, j); break;
+        }
+    }
+    if (!live) { cp_wait<0>(); return false; }
+    for (int j = 0; j < J; j += 4) {
+        body(IntC<0>{}, IntC<0>{}, j);
+        body(IntC<1>{}, IntC<0>{}, j + 1);
+        body(IntC<2>{}, IntC<0>{}, j + 2);
+        body(IntC<3>{}, IntC<0>{}, j + 3);
     }
     cp_wait<0>();
     return true;
@@ -291,16 +346,18 @@ __global__ void __launch_bounds__(kPrimalThreads, kCtasPerSm) k_primal(Sell KT, 
     PrimalSmem& P = *reinterpret_cast<PrimalSmem*>(smem_raw);
     dd* const red = P.red;
     grid_launch_dependents();
+    UC_TL_MARK(V, 0);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     dd acc[1] = {dd{0.0, 0.0}};
     const Policies pol{policy_evict_first(), policy_evict_last()};
     // everything below is set by dep_ready(), i.e. read after the previous kernel has completed
     int pend = 0; double eta_prev = 0.0, tau = 0.0;
     const double* xcur = nullptr; const double* ycur = nullptr; double* xnext = nullptr;
-    const double* vsrc[3]; int voff[3]; bool vok[3];   // this lane's share of a slice's vector segments: piece k covers
-                                                       // vector v = 2k + lane/16, doubles off, off+1
+    const double* vsrc[3]; int voff[3]; int vkey[3];   // this lane's share of a slice's vector segments: piece k covers
+                                                       // vector v = 2k + lane/16, doubles off, off+1; vkey 0: copy it
     auto dep_ready = [&]() -> bool {
         grid_dependency_wait();
+        UC_TL_MARK(V, 1);
         const CtrlHot h = load_hot(ctl);
         if (h.done) return false;
         const int cur = h.cur;
@@ -310,7 +367,7 @@ __global__ void __launch_bounds__(kPrimalThreads, kCtasPerSm) k_primal(Sell KT, 
         for (int k = 0; k < 3; ++k) {
             const int v = 2 * k + (lane >> 4), off = (lane & 15) * 2;
             vsrc[k] = (v == 0 ? xcur : v == 1 ? V.c : v == 2 ? V.l : v == 3 ? V.u : V.xsum) + off;
-            voff[k] = v * 32 + off; vok[k] = v < 4 || (v == 4 && pend);
+            voff[k] = v * 32 + off; vkey[k] = (v < 4 || (v == 4 && pend)) ? 0 : 1;
         }
         return true;
     };
@@ -328,9 +385,9 @@ __global__ void __launch_bounds__(kPrimalThreads, kCtasPerSm) k_primal(Sell KT, 
     } else {                                               // ---- consumer warps
         double g[1] = {0.0};
         const bool live = warp_pipeline(KT, P.w[warp], (int)blockIdx.x * kPrimalWarps + warp, lane, ycur, pol.first, dep_ready,
-            [&](auto& D, int row0, bool on) {              // x, c, l, u (, xsum): 16 pieces of 16 bytes each
+            [&](auto& D, int row0, int last01) {           // x, c, l, u (, xsum): 16 pieces of 16 bytes each
 #pragma unroll
-                for (int k = 0; k < 3; ++k) cp_stream16_if(on && vok[k], &D.vec[0][0] + voff[k], vsrc[k] + row0, pol.first);
+                for (int k = 0; k < 3; ++k) cp_stream16_lt(vkey[k], last01, &D.vec[0][0] + voff[k], vsrc[k] + row0, pol.first);
             },
             [&](auto& D, int info, int row0) {
                 if (info & kStepFirst) g[0] = 0.0;
@@ -345,8 +402,10 @@ __global__ void __launch_bounds__(kPrimalThreads, kCtasPerSm) k_primal(Sell KT, 
             });
         if (!live) return;
     }
-    block_sum_dd<1>(acc, red);
-    if (threadIdx.x == 0) V.partA[blockIdx.x] = acc[0];
+    UC_TL_MARK(V, 2);
+    if (!block_sum_dd_warp0<1>(acc, red)) return;           // the other warps leave; warp 0 finishes the CTA's partial
+    if (lane == 0) V.partA[blockIdx.x] = acc[0];
+    UC_TL_MARK(V, 3);
 }
 
 // ------------------------------------------------------------ A7+A8+A9 (+A10): dual kernel
@@ -366,6 +425,7 @@ __global__ void __launch_bounds__(kDualThreads, kCtasPerSm) k_dual(Sell K, Vecs 
     DualSmem& P = *reinterpret_cast<DualSmem*>(smem_raw);
     dd* const red = P.red;
     grid_launch_dependents();
+    UC_TL_MARK(V, 0);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     dd acc[2] = {dd{0.0, 0.0}, dd{0.0, 0.0}};
     const Policies pol{policy_evict_first(), policy_evict_last()};
@@ -373,7 +433,8 @@ __global__ void __launch_bounds__(kDualThreads, kCtasPerSm) k_dual(Sell K, Vecs 
     // everything below is set by dep_ready(), i.e. read after the previous kernel has completed
     int cur = 0, pend = 0; double eta_prev = 0.0, sig = 0.0;
     const double* ycur = nullptr; double* ynext = nullptr;
-    const double* vsrc[2]; int voff[2]; bool vok[2];   // this lane's share of a slice's vector segments
+    const double* vsrc[2]; int voff[2]; int vkey[2];   // this lane's share of a slice's vector segments (vkey 0: copy it)
+    const int bkey = (lane == 16 || lane == 17) ? 0 : 1;
     // inputs of the step rule (A9), fetched by one thread of every CTA while the kernel starts and parked in shared
     // memory: whichever CTA finishes last then runs the rule without a single cold load on the critical path of the
     // whole solve
@@ -381,6 +442,7 @@ __global__ void __launch_bounds__(kDualThreads, kCtasPerSm) k_dual(Sell K, Vecs 
     __shared__ RuleIn rule_in;
     auto dep_ready = [&]() -> bool {
         grid_dependency_wait();
+        UC_TL_MARK(V, 1);
         const CtrlHot h = load_hot(ctl);
         if (h.done) return false;
         cur = h.cur; pend = h.pending; eta_prev = h.eta_prev; sig = h.eta * h.omega;
@@ -395,7 +457,7 @@ __global__ void __launch_bounds__(kDualThreads, kCtasPerSm) k_dual(Sell K, Vecs 
         for (int k = 0; k < 2; ++k) {
             const int v = 2 * k + (lane >> 4), off = (lane & 15) * 2;
             vsrc[k] = (v == 0 ? ycur : v == 1 ? V.q : V.ysum) + off;
-            voff[k] = v * 32 + off; vok[k] = v < 2 || (v == 2 && pend);
+            voff[k] = v * 32 + off; vkey[k] = (v < 2 || (v == 2 && pend)) ? 0 : 1;
         }
         return true;
     };
@@ -417,10 +479,10 @@ __global__ void __launch_bounds__(kDualThreads, kCtasPerSm) k_dual(Sell K, Vecs 
     } else {                                               // ---- consumer warps
         double kx[2] = {0.0, 0.0};
         const bool live = warp_pipeline(K, P.w[warp], (int)blockIdx.x * kDualWarps + warp, lane, xg, pol.first, dep_ready,
-            [&](auto& D, int row0, bool on) {              // y, q (, ysum): 16 pieces each; isG: 2 pieces
+            [&](auto& D, int row0, int last01) {           // y, q (, ysum): 16 pieces each; isG: 2 pieces
 #pragma unroll
-                for (int k = 0; k < 2; ++k) cp_stream16_if(on && vok[k], &D.vec[0][0] + voff[k], vsrc[k] + row0, pol.first);
-                cp_stream16_if(on && (lane == 16 || lane == 17), &D.bvec[(lane & 1) * 16], V.isG + row0 + (lane & 1) * 16, pol.first);
+                for (int k = 0; k < 2; ++k) cp_stream16_lt(vkey[k], last01, &D.vec[0][0] + voff[k], vsrc[k] + row0, pol.first);
+                cp_stream16_lt(bkey, last01, &D.bvec[(lane & 1) * 16], V.isG + row0 + (lane & 1) * 16, pol.first);
             },
             [&](auto& D, int info, int row0) {
                 if (info & kStepFirst) { kx[0] = 0.0; kx[1] = 0.0; }
@@ -436,40 +498,49 @@ __global__ void __launch_bounds__(kDualThreads, kCtasPerSm) k_dual(Sell K, Vecs 
             });
         if (!live) return;
     }
-    block_sum_dd<2>(acc, red);
+    UC_TL_MARK(V, 2);
     // ---- A9: the last CTA finishes the reductions and runs the step-size rule (R5).  This is the serial tail of
-    // every attempt (measured: 8.6 us of 88 on config 3, 6.2 of 16 on config 1, before this form), so it is ONE warp,
-    // shuffles only, no block barrier, no cold load: the other warps are gone as soon as the block sum is done.
-    if (warp != 0) return;
+    // every attempt (timeline of profiles/r02b: 6.7 us of 85 on config 3 before this form), so it is ONE warp, with every
+    // wait it contains taken once: the other warps only arrive at the block barrier and leave; the CTA's partials are
+    // published by the release half of the ticket (no separate fence); the last CTA's warp fetches all partials of all
+    // CTAs in one round trip before it adds any; no cold load: the rule's inputs were parked in shared memory.
+    if (!block_sum_dd_warp0<2>(acc, red)) return;
+    UC_TL_MARK(V, 3);
     unsigned last = 0;
     if (lane == 0) {
         V.partB[blockIdx.x] = acc[0]; V.partB[V.gridPB + blockIdx.x] = acc[1];
-        __threadfence();
-        last = atomicAdd(&ctl->ticket_b, 1u) == gridDim.x - 1;
+        unsigned old;
+        asm volatile("atom.add.acq_rel.gpu.global.u32 %0, [%1], 1;" : "=r"(old) : "l"(&ctl->ticket_b) : "memory");
+        last = old == gridDim.x - 1;
     }
+    UC_TL_MARK(V, 4);
     if (!__shfl_sync(0xffffffffu, last, 0)) return;
-    __threadfence();
     dd s3[3] = {dd{0.0, 0.0}, dd{0.0, 0.0}, dd{0.0, 0.0}};
-    for (int i = lane; i < V.gridPA; i += 32) {
-        dd t; t.hi = __ldcg(&V.partA[i].hi); t.lo = __ldcg(&V.partA[i].lo);
-        s3[0] = dd_add(s3[0], t);
-    }
-    for (int i = lane; i < V.gridPB; i += 32) {
-        dd t, u;
-        t.hi = __ldcg(&V.partB[i].hi); t.lo = __ldcg(&V.partB[i].lo);
-        u.hi = __ldcg(&V.partB[V.gridPB + i].hi); u.lo = __ldcg(&V.partB[V.gridPB + i].lo);
-        s3[1] = dd_add(s3[1], t); s3[2] = dd_add(s3[2], u);
-    }
+    {
+        constexpr int U = 5;                              // 5 x 32 >= the 148 CTAs of a B200: one batch, one round trip
+        const double2* pa = reinterpret_cast<const double2*>(V.partA);
+        const double2* pb = reinterpret_cast<const double2*>(V.partB);
+        const int ga = V.gridPA, gb = V.gridPB, gmax = ga > gb ? ga : gb;
+        for (int base = 0; base < gmax; base += 32 * U) {
+            double2 ta[U], tb[U], tc[U];
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {                    // three independent chains per round: they interleave
+            for (int u = 0; u < U; ++u) {
+                const int i = base + u * 32 + lane;
+                ta[u] = i < ga ? __ldcg(pa + i) : make_double2(0.0, 0.0);
+                tb[u] = i < gb ? __ldcg(pb + i) : make_double2(0.0, 0.0);
+                tc[u] = i < gb ? __ldcg(pb + gb + i) : make_double2(0.0, 0.0);
+            }
 #pragma unroll
-        for (int q = 0; q < 3; ++q) {
-            dd t;
-            t.hi = __shfl_xor_sync(0xffffffffu, s3[q].hi, o);
-            t.lo = __shfl_xor_sync(0xffffffffu, s3[q].lo, o);
-            s3[q] = dd_add(s3[q], t);
+            for (int u = 0; u < U; ++u) {
+                s3[0] = dd_add(s3[0], dd{ta[u].x, ta[u].y});
+                s3[1] = dd_add(s3[1], dd{tb[u].x, tb[u].y});
+                s3[2] = dd_add(s3[2], dd{tc[u].x, tc[u].y});
+            }
         }
     }
+    UC_TL_MARK(V, 5);
+    warp_sum_dd_n<3>(s3);
+    UC_TL_MARK(V, 6);
     if (lane != 0) return;
     ctl->ticket_b = 0;
     const double dx2 = dd_round(s3[0]), dy2 = dd_round(s3[1]), inter = fabs(dd_round(s3[2]));
@@ -495,6 +566,7 @@ __global__ void __launch_bounds__(kDualThreads, kCtasPerSm) k_dual(Sell K, Vecs 
     ctl->eta = eta_next;
     ctl->k = k;
     if (!isfinite(eta_next) || !(eta_next > 0.0)) { ctl->status = UC_NUMERICAL_ERROR; ctl->done = 1; }
+    UC_TL_MARK(V, 3);                        // the warp that ran the step rule: when the attempt was decided
 }
 
 }  // namespace ucpdhg

@@ -73,31 +73,51 @@ struct HostSell {
     int64_t steps_per_warp = 0, sched_warps = 0;
 };
 
-// Static schedule of the persistent attempt kernels for `warps` consumer warps in total.  Slices are taken in
-// ascending order and each goes to the warp with the least estimated work so far (ties: lowest warp), so that
-// the warps finish together while, at any moment, all warps work on neighbouring slices (DRAM pages and L2
-// lines are shared).  The estimate is in units of ~100 cycles from the measured per-step breakdown
-// (DESIGN.md section 7): 7 per step + 1.3 per entry per row + 4 for the step that applies the update.  A warp takes its slices in ascending order, each as
-// ceil(width / kChunkT) steps.  Stored step-major, steps[j * warps + w], padded with empty steps to the
-// longest warp, so that step j of all warps is one coalesced read.  The assignment is fixed at create time:
-// solves are reproducible bit for bit.
-inline void build_schedule(HostSell& S, int64_t warps) {
-    if (warps < 1) warps = 1;
+// Static schedule of the persistent attempt kernels for `ctas` CTAs of `warps_per_cta` consumer warps.
+//   1. The slices are cut into `ctas` CONTIGUOUS ranges of (nearly) equal estimated cost, one per CTA: the gathers of
+//      neighbouring rows fall into the same few blocks of the gathered vector (in a UC LP: the rows / variables of one
+//      period), so a CTA that sweeps a contiguous range finds most gathered sectors in ITS L1 -- the attempt kernels
+//      are bound by L2 sector throughput (~6300 B/cycle chip-wide), of which scattered 8/16-byte gathers, each pulling
+//      a 32-byte sector, were half (profiles/r02b).
+//   2. Inside its range a CTA deals the slices, in ascending order, to its warp with the least estimated work so far
+//      (ties: lowest warp), so that its warps finish together while, at any moment, they work on neighbouring slices
+//      (one shared working set in L1).
+// The estimate is in units of ~100 cycles from the measured per-step breakdown: 7 per step +
+// 1.3 per entry per row + 4 for the step that applies the update.  A warp takes its slices in ascending order, each as
+// ceil(width / kChunkT) steps.  Stored step-major, steps[j * warps + w] with w = cta * warps_per_cta + warp, padded with
+// empty steps to the longest warp, so that step j of all warps is one coalesced read.  The assignment is fixed at
+// create time: solves are reproducible bit for bit.
+inline int64_t slice_cost(int64_t wd) {
+    const int64_t nch = std::max<int64_t>(1, (wd + kChunkT - 1) / kChunkT);
+    return 70 * nch + 13 * wd + 40;
+}
+inline void build_schedule(HostSell& S, int64_t ctas, int64_t warps_per_cta) {
+    if (ctas < 1) ctas = 1;
+    if (warps_per_cta < 1) warps_per_cta = 1;
+    const int64_t warps = ctas * warps_per_cta;
     S.sched_warps = warps;
     std::vector<int32_t> owner((size_t)S.nslices);
     std::vector<int64_t> count((size_t)warps, 0);
     {
-        typedef std::pair<int64_t, int64_t> Load;                    // (steps so far, warp)
-        std::priority_queue<Load, std::vector<Load>, std::greater<Load>> heap;
-        for (int64_t w = 0; w < warps; ++w) heap.push(Load(0, w));
-        for (int64_t s = 0; s < S.nslices; ++s) {
-            const int64_t wd = (S.slice_ptr[(size_t)s + 1] - S.slice_ptr[(size_t)s]) / 32;
-            Load l = heap.top(); heap.pop();
-            owner[(size_t)s] = (int32_t)l.second;
-            const int64_t nch = std::max<int64_t>(1, (wd + kChunkT - 1) / kChunkT);
-            l.first += 70 * nch + 13 * wd + 40;
-            count[(size_t)l.second] += nch;
-            heap.push(l);
+        std::vector<int64_t> wd((size_t)S.nslices);
+        int64_t total = 0;
+        for (int64_t s = 0; s < S.nslices; ++s) { wd[(size_t)s] = (S.slice_ptr[(size_t)s + 1] - S.slice_ptr[(size_t)s]) / 32; total += slice_cost(wd[(size_t)s]); }
+        typedef std::pair<int64_t, int64_t> Load;                    // (work so far, warp)
+        int64_t s = 0, done = 0;
+        for (int64_t c = 0; c < ctas; ++c) {
+            // range of CTA c: up to the slice where the running cost passes (c + 1) / ctas of the total
+            const int64_t target = (total * (c + 1)) / ctas;
+            std::priority_queue<Load, std::vector<Load>, std::greater<Load>> heap;
+            for (int64_t w = 0; w < warps_per_cta; ++w) heap.push(Load(0, c * warps_per_cta + w));
+            while (s < S.nslices && (c == ctas - 1 || done + slice_cost(wd[(size_t)s]) / 2 <= target)) {
+                Load l = heap.top(); heap.pop();
+                owner[(size_t)s] = (int32_t)l.second;
+                l.first += slice_cost(wd[(size_t)s]);
+                done += slice_cost(wd[(size_t)s]);
+                count[(size_t)l.second] += std::max<int64_t>(1, (wd[(size_t)s] + kChunkT - 1) / kChunkT);
+                heap.push(l);
+                ++s;
+            }
         }
     }
     int64_t J = 0;

@@ -108,7 +108,21 @@ struct Vecs {
     int gridA, gridB, gridR;     // grids of the check kernels (persistent: grid-stride over the layout's blocks) and of
                                  // the one-thread-per-element restart / flush kernels
     int gridPA, gridPB;          // persistent grids of the two attempt kernels
+#ifdef UC_TIMELINE
+    unsigned long long* tl;      // [grid][kTlWarps][kTlMarks] globaltimer marks of the kernel being launched (measurement build only)
+#endif
 };
+// -DUC_TIMELINE (measurement build, uc_pdhg_timeline): every warp of the attempt kernels records when it entered the
+// kernel, when its grid dependency resolved, when it finished its steps and when it left.
+constexpr int kTlWarps = 32, kTlMarks = 8;
+#ifdef UC_TIMELINE
+__device__ __forceinline__ unsigned long long tl_now() { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
+#define UC_TL_MARK(V, i)                                                                                               \
+    do { if ((V).tl && (threadIdx.x & 31) == 0)                                                                        \
+        (V).tl[((size_t)blockIdx.x * kTlWarps + (threadIdx.x >> 5)) * kTlMarks + (i)] = tl_now(); } while (0)
+#else
+#define UC_TL_MARK(V, i) do { } while (0)
+#endif
 
 // ------------------------------------------------------------------------------------------ loads
 __device__ __forceinline__ double ld_stream(const double* p) {   // read-once data: keep it out of L1
@@ -167,6 +181,39 @@ __device__ __forceinline__ void block_sum_dd(dd (&v)[NV], dd* red) {
         for (int q = 0; q < NV; ++q) v[q] = red[q * 32];
     }
     __syncthreads();
+}
+
+// The same sums when only warp 0 needs them (the attempt kernels: this is the serial tail of every attempt).  Every warp
+// reduces its own values by shuffles (the NV chains interleave), parks them in shared memory and ARRIVES at named
+// barrier 1 -- it does not wait and is free to leave the kernel; warp 0 waits for all arrivals and adds the per-warp
+// results.  Returns true in warp 0 (result in every lane of it), false elsewhere.  red: NV * 32 dd.
+template <int NV>
+__device__ __forceinline__ void warp_sum_dd_n(dd (&v)[NV]) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+        for (int q = 0; q < NV; ++q) {
+            dd t;
+            t.hi = __shfl_xor_sync(0xffffffffu, v[q].hi, o);
+            t.lo = __shfl_xor_sync(0xffffffffu, v[q].lo, o);
+            v[q] = dd_add(v[q], t);
+        }
+    }
+}
+template <int NV>
+__device__ __forceinline__ bool block_sum_dd_warp0(dd (&v)[NV], dd* red) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+    warp_sum_dd_n<NV>(v);
+    if (lane == 0) {
+#pragma unroll
+        for (int q = 0; q < NV; ++q) red[q * 32 + warp] = v[q];
+    }
+    if (warp != 0) { asm volatile("bar.arrive 1, %0;" ::"r"(nw * 32) : "memory"); return false; }
+    asm volatile("bar.sync 1, %0;" ::"r"(nw * 32) : "memory");
+#pragma unroll
+    for (int q = 0; q < NV; ++q) v[q] = lane < nw ? red[q * 32 + lane] : dd{0.0, 0.0};
+    warp_sum_dd_n<NV>(v);
+    return true;
 }
 
 // double-double sums of NV partial arrays (part + q * stride, `count` entries each) by one block, in one pass;

@@ -225,8 +225,16 @@ void launch_pdl(Kern kern, int grid, int threads, size_t smem, cudaStream_t st, 
     cfg.attrs = attr; cfg.numAttrs = 1;
     CK(cudaLaunchKernelEx(&cfg, kern, A, V, ctl));
 }
-void launch_primal(uc_lp* lp, cudaStream_t st) { launch_pdl(k_primal, lp->V.gridPA, kPrimalThreads, kPrimalSmemBytes, st, lp->KT, lp->V, lp->ctl); }
-void launch_dual(uc_lp* lp, cudaStream_t st) { launch_pdl(k_dual, lp->V.gridPB, kDualThreads, kDualSmemBytes, st, lp->K, lp->V, lp->ctl); }
+// Both attempt kernels ask for the SAME amount of dynamic shared memory, so that an SM never changes its L1 / shared
+// memory split between them (the two alternate ~20,000 times per second)
+#ifdef UC_SMEM_REQUEST
+constexpr size_t kAttemptSmemBytes = UC_SMEM_REQUEST;
+#else
+constexpr size_t kAttemptSmemBytes = kPrimalSmemBytes > kDualSmemBytes ? kPrimalSmemBytes : kDualSmemBytes;
+#endif
+static_assert(kAttemptSmemBytes >= kPrimalSmemBytes && kAttemptSmemBytes >= kDualSmemBytes, "shared memory request");
+void launch_primal(uc_lp* lp, cudaStream_t st) { launch_pdl(k_primal, lp->V.gridPA, kPrimalThreads, kAttemptSmemBytes, st, lp->KT, lp->V, lp->ctl); }
+void launch_dual(uc_lp* lp, cudaStream_t st) { launch_pdl(k_dual, lp->V.gridPB, kDualThreads, kAttemptSmemBytes, st, lp->K, lp->V, lp->ctl); }
 void launch_attempt(uc_lp* lp, cudaStream_t st) { launch_primal(lp, st); launch_dual(lp, st); }
 void launch_kkt(uc_lp* lp, cudaStream_t st, int mode) {
     const int flush = mode == kModeCheck;        // the periodic check also applies the pending average term (R6)
@@ -312,8 +320,8 @@ const char* uc_last_error(void) { return g_err.c_str(); }
 // exactly as uc_lp_create does and verifies them against the caller's CSR.  Returns UC_OK or UC_ERR_INVALID with
 // the first violated property in uc_last_error().
 int uc_host_layout_selftest(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, const int32_t* col_idx, const double* val,
-                            int32_t sell_window, int32_t long_row_threshold, int32_t sched_warps) {
-    if (m < 0 || n < 0 || nnz < 0 || !row_ptr || sell_window < 32 || long_row_threshold < 1 || sched_warps < 1)
+                            int32_t sell_window, int32_t long_row_threshold, int32_t sched_ctas, int32_t warps_per_cta) {
+    if (m < 0 || n < 0 || nnz < 0 || !row_ptr || sell_window < 32 || long_row_threshold < 1 || sched_ctas < 1 || warps_per_cta < 1)
         return fail(UC_ERR_INVALID, "bad argument");
     HostProblem P;
     build_perms(m, n, nnz, row_ptr, col_idx, sell_window, long_row_threshold, P);
@@ -321,8 +329,8 @@ int uc_host_layout_selftest(int64_t m, int64_t n, int64_t nnz, const int64_t* ro
     build_KT(row_ptr, col_idx, val, true, P);
     compress_columns(P.K, true);
     compress_columns(P.KT, true);
-    build_schedule(P.K, sched_warps);
-    build_schedule(P.KT, sched_warps);
+    build_schedule(P.K, sched_ctas, warps_per_cta);
+    build_schedule(P.KT, sched_ctas, warps_per_cta);
     auto bad = [&](const std::string& what) { return fail(UC_ERR_INVALID, what); };
     // ---- permutations: bijections, rows with <= threshold entries first, the others last in the caller's order
     auto check_perm = [&](const std::vector<int64_t>& perm, const std::vector<int64_t>& inv, int64_t N, int64_t nshort,
@@ -441,6 +449,23 @@ int uc_host_layout_selftest(int64_t m, int64_t n, int64_t nnz, const int64_t* ro
             }
         }
         for (int64_t sl = 0; sl < S.nslices; ++sl) if (done[(size_t)sl] != 1) return "slice not scheduled";
+        // ---- a CTA owns one contiguous range of slices, ranges in CTA order
+        if (W != (int64_t)sched_ctas * warps_per_cta) return "schedule width";
+        int64_t prev_hi = -1;
+        for (int64_t c = 0; c < sched_ctas; ++c) {
+            int64_t lo = S.nslices, hi = -1, cnt = 0;
+            for (int64_t wq = c * warps_per_cta; wq < (c + 1) * warps_per_cta; ++wq)
+                for (int64_t j = 0; j < J; ++j) {
+                    const StepDesc d = S.steps[(size_t)(j * W + wq)];
+                    if (!((d.w0 >> 26) & kStepFirst)) continue;
+                    const int64_t sl = d.row0 / 32;
+                    lo = std::min(lo, sl); hi = std::max(hi, sl); ++cnt;
+                }
+            if (cnt == 0) continue;
+            if (hi - lo + 1 != cnt) return "the slices of a CTA are not one contiguous range";
+            if (lo != prev_hi + 1) return "CTA ranges out of order";
+            prev_hi = hi;
+        }
         return "";
     };
     std::string w = check_sell(P.K, false);
@@ -521,7 +546,7 @@ int uc_lp_create(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, cons
                 build_K(row_ptr, col_idx, val, want_src, P);
                 if (P.K.col.size() >= (size_t)1 << 31) throw std::bad_alloc();   // step descriptors address entries / 32 in 26 bits
                 compress_columns(P.K, opt.index_compression != 0);
-                build_schedule(P.K, (int64_t)gridPB * kDualWarps);
+                build_schedule(P.K, gridPB, kDualWarps);
                 lp->K = upload_sell(lp, P.K);
             } catch (...) { k_side_error = std::current_exception(); }
         });
@@ -529,7 +554,7 @@ int uc_lp_create(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, cons
             build_KT(row_ptr, col_idx, val, want_src, P);
             if (P.KT.col.size() >= (size_t)1 << 31) throw std::bad_alloc();
             compress_columns(P.KT, opt.index_compression != 0);
-            build_schedule(P.KT, (int64_t)gridPA * kPrimalWarps);
+            build_schedule(P.KT, gridPA, kPrimalWarps);
             lp->KT = upload_sell(lp, P.KT);
         } catch (...) { k_side.join(); throw; }
         k_side.join();
@@ -560,8 +585,8 @@ int uc_lp_create(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, cons
             V.gridA = std::max(1, std::min(cap, lp->KT.grid)); V.gridB = std::max(1, std::min(cap, lp->K.grid));
         }
         V.gridPA = gridPA; V.gridPB = gridPB;
-        CK(cudaFuncSetAttribute(k_primal, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kPrimalSmemBytes));
-        CK(cudaFuncSetAttribute(k_dual, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kDualSmemBytes));
+        CK(cudaFuncSetAttribute(k_primal, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kAttemptSmemBytes));
+        CK(cudaFuncSetAttribute(k_dual, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kAttemptSmemBytes));
         V.partA = lp->dalloc<dd>((size_t)V.gridPA);
         V.partB = lp->dalloc<dd>((size_t)2 * V.gridPB);
         V.partD = lp->dalloc<dd>((size_t)8 * V.gridA);
@@ -904,6 +929,47 @@ int uc_pdhg_time_kernels(uc_lp* lp, void* stream, int32_t attempts, double* prim
     for (auto& e : ev) if (e) cudaEventDestroy(e);
     lp->busy.store(0);
     return rc;
+}
+
+int uc_pdhg_timeline(uc_lp* lp, void* stream, int32_t attempts, uint64_t* out, int64_t cap, int32_t* grid_primal, int32_t* grid_dual) {
+#ifndef UC_TIMELINE
+    (void)lp; (void)stream; (void)attempts; (void)out; (void)cap; (void)grid_primal; (void)grid_dual;
+    return fail(UC_ERR_INVALID, "this library was built without -DUC_TIMELINE");
+#else
+    if (!lp || attempts <= 0 || !out || !grid_primal || !grid_dual) return fail(UC_ERR_INVALID, "bad argument");
+    const int64_t need = (int64_t)(lp->V.gridPA + lp->V.gridPB) * kTlWarps * kTlMarks;
+    if (cap < need) return fail(UC_ERR_INVALID, "timeline buffer too small: need " + std::to_string(need) + " entries");
+    int expected = 0;
+    if (!lp->busy.compare_exchange_strong(expected, 1)) return fail(UC_ERR_BUSY, "a solve is running on this handle");
+    int rc = UC_OK;
+    unsigned long long* d = nullptr;
+    try {
+        DeviceGuard guard(lp->device);
+        cudaStream_t st = stream ? (cudaStream_t)stream : lp->own_stream;
+        uc_pdhg_params prm; uc_pdhg_default_params(&prm);
+        CK(cudaMalloc((void**)&d, sizeof(unsigned long long) * (size_t)need));
+        CK(cudaMemset(d, 0, sizeof(unsigned long long) * (size_t)need));
+        ensure_powtab(lp, (long long)attempts);
+        start_run(lp, prm, st, (long long)attempts, true, nullptr, nullptr, nullptr, nullptr);
+        // the marks of the LAST attempt survive; the dual block starts after the primal block
+        for (int i = 0; i < attempts; ++i) {
+            const bool last = i == attempts - 1;
+            lp->V.tl = last ? d : nullptr;
+            launch_primal(lp, st);
+            lp->V.tl = last ? d + (size_t)lp->V.gridPA * kTlWarps * kTlMarks : nullptr;
+            launch_dual(lp, st);
+        }
+        lp->V.tl = nullptr;
+        CK(cudaMemcpyAsync(out, d, sizeof(unsigned long long) * (size_t)need, cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        *grid_primal = lp->V.gridPA; *grid_dual = lp->V.gridPB;
+    } catch (const CudaFail& f) {
+        rc = fail(UC_ERR_CUDA, std::string(f.what) + ": " + cudaGetErrorString(f.e));
+    }
+    if (d) cudaFree(d);
+    lp->busy.store(0);
+    return rc;
+#endif
 }
 
 int uc_lp_get_info(const uc_lp* lp, uc_lp_info* info) {

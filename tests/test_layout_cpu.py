@@ -22,11 +22,12 @@ def test_layouts_and_schedules_reproduce_the_csr(name):
     B.host_layout_selftest(CASES[name]())
 
 
-@pytest.mark.parametrize("window,thr,warps", [(32, 1, 1), (64, 4, 7), (4096, 32, 15), (100000, 1000, 2220), (4096, 3, 148 * 15)])
-def test_layout_options_and_warp_counts(window, thr, warps):
-    """Tiny windows, every row long / no row long, more warps than slices, a single warp."""
-    for lp in (ragged_lp(), uc_config(0)):
-        B.host_layout_selftest(lp, sell_window=window, long_row_threshold=thr, sched_warps=warps)
+@pytest.mark.parametrize("window,thr,ctas,wpc", [(32, 1, 1, 1), (64, 4, 7, 1), (64, 4, 3, 5), (4096, 32, 1, 15), (100000, 1000, 148, 15),
+                                                 (4096, 3, 148, 15), (4096, 32, 296, 7)])
+def test_layout_options_and_warp_counts(window, thr, ctas, wpc):
+    """Tiny windows, every row long / no row long, more warps (and CTAs) than slices, a single warp."""
+    for lp in (ragged_lp(), uc_config(0), uc_config(1)):
+        B.host_layout_selftest(lp, sell_window=window, long_row_threshold=thr, sched_ctas=ctas, warps_per_cta=wpc)
 
 
 def banded_and_wide_lp(n=200_000, m=150_000, seed=4):
@@ -75,4 +76,6 @@ def test_bad_arguments_are_rejected():
     with pytest.raises(B.UcError):
         B.host_layout_selftest(lp, sell_window=8)
     with pytest.raises(B.UcError):
-        B.host_layout_selftest(lp, sched_warps=0)
+        B.host_layout_selftest(lp, sched_ctas=0)
+    with pytest.raises(B.UcError):
+        B.host_layout_selftest(lp, warps_per_cta=0)

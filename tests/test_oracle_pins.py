@@ -1,7 +1,8 @@
 """Pins for the CPU oracle (no GPU): each test checks oracle/ against something OTHER than itself --
 values printed in SURVEY.md 8(c) worked examples (tests/golden/), closed forms, brute-force vertex
 enumeration, HiGHS, dense numpy algebra, and textbook invariants of PDHG.  DESIGN.md lists which
-reading (R1..R14) each pin covers and which remain 'parity unpinned' (R10, R11 decisions)."""
+reading (R1..R14) each pin covers; none remains 'parity unpinned' (R10 / R11: the worked restart example and the
+dense replay of every restart decision below)."""
 import math
 
 import numpy as np
