@@ -64,6 +64,9 @@ typedef struct {
     int32_t index_compression;  /* 1 (default): slices whose column indices span < 2^16 store them as 16-bit offsets from
                                    the slice's smallest index (SURVEY.md 8(f) NEXT-4, 2 bytes per entry less per matrix
                                    copy; results are bit-identical); 0: 32-bit indices everywhere */
+    int32_t host_ingest;        /* 0 (default): step A1 -- permutations, explicit transpose, both layouts -- runs as kernels on
+                                   the device from one copy of the caller's CSR; 1: the host builders (the checker's code)
+                                   build them and upload.  Both give the same layouts bit for bit (uc_lp_compare_layout) */
 } uc_lp_options;
 
 void uc_lp_default_options(uc_lp_options* opt);
@@ -217,8 +220,10 @@ int uc_lp_get_scaling(uc_lp* lp, double* Dr_out, double* Dc_out);
    for R1 and for "K' equals the CSC of K bit-exactly". */
 int uc_lp_get_scaled_values(uc_lp* lp, int32_t from_transpose, double* val_out);
 
-/* out = Ktilde v (transpose = 0; v[n], out[m]) or Ktilde' v (transpose = 1; v[m], out[n]) with the
-   solver's own SpMV kernels; HOST in/out, original order.  Test hook for the adjoint identity. */
+/* out = Ktilde v (transpose = 0; v[n], out[m]) or Ktilde' v (transpose = 1; v[m], out[n]) over the handle's own layouts
+   with the row traversal of the CHECK kernels (A11); HOST in/out, original order.  Test hook for the layouts and the
+   adjoint identity.  (The pipelines of the attempt kernels are covered by the one-attempt test of
+   tests/test_gpu_parity.py, which runs k_primal + k_dual once from a warm start through uc_pdhg_solve.) */
 int uc_lp_spmv(uc_lp* lp, int32_t transpose, const double* v, double* out);
 
 /* Host-only self-check of ingest step A1 (no GPU needed): builds the row / column permutations, the explicit
@@ -229,6 +234,13 @@ int uc_lp_spmv(uc_lp* lp, int32_t transpose, const double* v, double* out);
    Returns UC_OK, or UC_ERR_INVALID with the violated property in uc_last_error(). */
 int uc_host_layout_selftest(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, const int32_t* col_idx, const double* val,
                             int32_t sell_window, int32_t long_row_threshold, int32_t sched_ctas, int32_t warps_per_cta);
+
+/* Test hook for ingest step A1 (needs the GPU): rebuilds the permutations, both layouts (16-bit offsets included) and both
+   attempt schedules from the caller's CSR with the HOST builders that uc_host_layout_selftest verifies, downloads what
+   the handle holds on the device and compares bit for bit (the matrix values only if the handle was created with
+   ruiz_iters = 0 and pc_alpha = 0: uc_lp_create scales them in place).  UC_OK, or UC_ERR_INVALID naming the first
+   difference.  With host_ingest = 0 this is the parity test of the device-side ingest kernels. */
+int uc_lp_compare_layout(uc_lp* lp, int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, const int32_t* col_idx, const double* val);
 
 /* Host evaluation of the double-double log / exp that the primal-weight update (R11) runs on the
    device (same source, csrc/uc_dd.cuh).  Test hooks: no GPU needed. */

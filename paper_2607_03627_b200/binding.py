@@ -22,7 +22,7 @@ class UcError(RuntimeError):
 class Options(C.Structure):
     _fields_ = [("device", C.c_int32), ("ruiz_iters", C.c_int32), ("pc_alpha", C.c_double),
                 ("sell_window", C.c_int32), ("long_row_threshold", C.c_int32),
-                ("keep_source_map", C.c_int32), ("index_compression", C.c_int32)]
+                ("keep_source_map", C.c_int32), ("index_compression", C.c_int32), ("host_ingest", C.c_int32)]
 
 
 class Params(C.Structure):
@@ -60,7 +60,7 @@ CHECK_DTYPE = np.dtype([("k", "i8"), ("restart_kind", "i4"), ("candidate", "i4")
                         ("mu_c", "f8"), ("mu_r", "f8"), ("relkkt_cur", "f8"), ("relkkt_avg", "f8")])
 
 EXPORTS = ["uc_lp_default_options", "uc_lp_create", "uc_lp_update_bounds", "uc_lp_update_objective", "uc_lp_destroy",
-           "uc_pdhg_default_params", "uc_pdhg_solve", "uc_pdhg_solve_device", "uc_pdhg_solve_batch", "uc_pdhg_cancel", "uc_pdhg_time_kernels", "uc_pdhg_timeline",
+           "uc_pdhg_default_params", "uc_pdhg_solve", "uc_pdhg_solve_device", "uc_pdhg_solve_batch", "uc_pdhg_cancel", "uc_pdhg_time_kernels", "uc_pdhg_timeline", "uc_lp_compare_layout",
            "uc_lp_get_info", "uc_lp_get_scaling", "uc_lp_get_scaled_values", "uc_lp_spmv", "uc_last_error",
            "uc_host_log_rounded", "uc_host_exp_rounded", "uc_host_layout_selftest"]
 
@@ -240,6 +240,15 @@ class UcLp:
         _check(self.lib.uc_lp_update_objective(self._h, cp))
 
     update_objective = uc_lp_update_objective
+
+    def uc_lp_compare_layout(self, lp):
+        """Raises UcError unless the device holds, bit for bit, the layouts the host builders make of `lp` (the LP it was created from)."""
+        rp = np.ascontiguousarray(lp.row_ptr, dtype=np.int64); ci = np.ascontiguousarray(lp.col_idx, dtype=np.int32)
+        va = np.ascontiguousarray(lp.val, dtype=np.float64)
+        _check(self.lib.uc_lp_compare_layout(self._h, C.c_int64(self.m), C.c_int64(self.n), C.c_int64(self.nnz), C.c_void_p(rp.ctypes.data),
+                                             C.c_void_p(ci.ctypes.data), C.c_void_p(va.ctypes.data)))
+
+    compare_layout = uc_lp_compare_layout
 
     def uc_pdhg_time_kernels(self, attempts=64, stream=None):
         """(primal_ms, dual_ms): average device time of the two kernels of an attempt (CUDA events)."""

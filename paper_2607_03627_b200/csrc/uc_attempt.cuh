@@ -55,7 +55,13 @@ namespace ucpdhg {
 #ifndef UC_DB
 #define UC_DB 1
 #endif
-constexpr int kPrimalWarps = UC_PRIMAL_WARPS, kDualWarps = UC_DUAL_WARPS;      // consumer warps per CTA
+#ifndef UC_MIN_WARPS
+#define UC_MIN_WARPS 4
+#endif
+// consumer warps per CTA: the most a CTA may have (the rings of that many are laid out in shared memory).  A handle
+// launches fewer when its LP has fewer than #SM x that many slices (uc_lp_create: attempt_shape), down to kMinWarps: on
+// small LPs a warp has one slice or none, and every extra warp only lengthens the block barrier of the serial tail.
+constexpr int kPrimalWarps = UC_PRIMAL_WARPS, kDualWarps = UC_DUAL_WARPS, kMinWarps = UC_MIN_WARPS;
 constexpr int kCtasPerSm = UC_CTAS_PER_SM;
 constexpr int kPrimalThreads = (kPrimalWarps + 1) * 32, kDualThreads = (kDualWarps + 1) * 32;   // + long-row warp
 // pipeline depth, per kernel: data (values, vectors, gathers) run kDB steps ahead of the compute, indices
@@ -237,6 +243,8 @@ __device__ __forceinline__ bool warp_pipeline(const Sell& A, Ring& R, int gw, in
             if (info_a & kStepEnd) J = min(J, sa);
             q_info[qa] = info_a; q_row[qa] = row_a; q_cb[qa] = cb_a < 0 ? 0 : cb_a; q_eb[qa] = eb32;
             const long long e0 = ((long long)eb32 << 5) + lane;
+            UC_BOUNDS_ASSERT(nt <= kChunkT && ((long long)eb32 << 5) + 32LL * nt <= A.nslots && row_a >= 0 && row_a <= A.nshort + 31 && (row_a & 31) == 0);
+            UC_BOUNDS_ASSERT(nt == 0 || (cb_a >= 0 ? A.col16 != nullptr : A.col != nullptr));
             if (cb_a >= 0) {
                 const unsigned short* p = A.col16 + e0;
 #pragma unroll
@@ -262,11 +270,10 @@ __device__ __forceinline__ bool warp_pipeline(const Sell& A, Ring& R, int gw, in
             issue_vecs(D, row_b, (info_b >> 4) & 1);               // kStepLast
             const GT* gs = gsrc + q_cb[qb];
 #pragma unroll
-#ifdef UC_EXP_COALESCED
-            for (int t = 0; t < kChunkT; ++t) cp_gather_lt(t, nt, &D.gv[t * 32 + lane], gsrc + (row_b / 2 + 32 * t + lane));
-#else
-            for (int t = 0; t < kChunkT; ++t) cp_gather_lt(t, nt, &D.gv[t * 32 + lane], gs + q_idx[qb][t]);
-#endif
+            for (int t = 0; t < kChunkT; ++t) {
+                UC_BOUNDS_ASSERT(t >= nt || (q_cb[qb] + q_idx[qb][t] >= 0 && (long long)q_cb[qb] + q_idx[qb][t] < A.ncols));
+                cp_gather_lt(t, nt, &D.gv[t * 32 + lane], gs + q_idx[qb][t]);
+            }
             c_info[db] = info_b; c_row[db] = row_b;
             cp_commit();
         }
@@ -372,7 +379,7 @@ __global__ void __launch_bounds__(kPrimalThreads, kCtasPerSm) k_primal(Sell KT, 
         return true;
     };
 
-    if (warp == kPrimalWarps) {                               // ---- long rows, one per pass
+    if (warp == KT.cta_warps) {                               // ---- long rows, one per pass
         if (!dep_ready()) return;
         for (int r = blockIdx.x; r < KT.nlong; r += gridDim.x) {
             const long long j = KT.nshort + r;
@@ -384,7 +391,7 @@ __global__ void __launch_bounds__(kPrimalThreads, kCtasPerSm) k_primal(Sell KT, 
         }
     } else {                                               // ---- consumer warps
         double g[1] = {0.0};
-        const bool live = warp_pipeline(KT, P.w[warp], (int)blockIdx.x * kPrimalWarps + warp, lane, ycur, pol.first, dep_ready,
+        const bool live = warp_pipeline(KT, P.w[warp], (int)blockIdx.x * KT.cta_warps + warp, lane, ycur, pol.first, dep_ready,
             [&](auto& D, int row0, int last01) {           // x, c, l, u (, xsum): 16 pieces of 16 bytes each
 #pragma unroll
                 for (int k = 0; k < 3; ++k) cp_stream16_lt(vkey[k], last01, &D.vec[0][0] + voff[k], vsrc[k] + row0, pol.first);
@@ -446,7 +453,7 @@ __global__ void __launch_bounds__(kDualThreads, kCtasPerSm) k_dual(Sell K, Vecs 
         const CtrlHot h = load_hot(ctl);
         if (h.done) return false;
         cur = h.cur; pend = h.pending; eta_prev = h.eta_prev; sig = h.eta * h.omega;
-        if (threadIdx.x == kDualWarps * 32) {              // the long-row warp: its dependent loads delay no slice
+        if (threadIdx.x == K.cta_warps * 32) {             // the long-row warp: its dependent loads delay no slice
             RuleIn r;
             r.eta = h.eta; r.omega = h.omega; r.w = h.w; r.k = ctl->k; r.acc = ctl->accepted;
             r.att = ctl->att; r.cap = ctl->att_cap; r.pw = ctl->powtab[r.k];     // {(k+1)^-0.6, (k+1)^-0.3} of attempt k = r.k + 1
@@ -462,7 +469,7 @@ __global__ void __launch_bounds__(kDualThreads, kCtasPerSm) k_dual(Sell K, Vecs 
         return true;
     };
 
-    if (warp == kDualWarps) {                               // ---- long rows
+    if (warp == K.cta_warps) {                              // ---- long rows
         if (!dep_ready()) return;
         auto gather = [&](int c, double (&o)[2]) { const double2 t = __ldg(xg + c); o[0] = t.x; o[1] = t.y; };
         for (int r = blockIdx.x; r < K.nlong; r += gridDim.x) {
@@ -478,7 +485,7 @@ __global__ void __launch_bounds__(kDualThreads, kCtasPerSm) k_dual(Sell K, Vecs 
         }
     } else {                                               // ---- consumer warps
         double kx[2] = {0.0, 0.0};
-        const bool live = warp_pipeline(K, P.w[warp], (int)blockIdx.x * kDualWarps + warp, lane, xg, pol.first, dep_ready,
+        const bool live = warp_pipeline(K, P.w[warp], (int)blockIdx.x * K.cta_warps + warp, lane, xg, pol.first, dep_ready,
             [&](auto& D, int row0, int last01) {           // y, q (, ysum): 16 pieces each; isG: 2 pieces
 #pragma unroll
                 for (int k = 0; k < 2; ++k) cp_stream16_lt(vkey[k], last01, &D.vec[0][0] + voff[k], vsrc[k] + row0, pol.first);
@@ -532,9 +539,9 @@ __global__ void __launch_bounds__(kDualThreads, kCtasPerSm) k_dual(Sell K, Vecs 
             }
 #pragma unroll
             for (int u = 0; u < U; ++u) {
-                s3[0] = dd_add(s3[0], dd{ta[u].x, ta[u].y});
-                s3[1] = dd_add(s3[1], dd{tb[u].x, tb[u].y});
-                s3[2] = dd_add(s3[2], dd{tc[u].x, tc[u].y});
+                s3[0] = dd_acc(s3[0], dd{ta[u].x, ta[u].y});
+                s3[1] = dd_acc(s3[1], dd{tb[u].x, tb[u].y});
+                s3[2] = dd_acc(s3[2], dd{tc[u].x, tc[u].y});
             }
         }
     }

@@ -41,6 +41,17 @@ __host__ __device__ __forceinline__ dd dd_add_d(dd a, double b) {
     dd s = two_sum(a.hi, b);
     s.lo += a.lo; return quick_two_sum(s.hi, s.lo);
 }
+// Cascaded addition for the SERIAL TAIL of an attempt (the reductions between the last row and the step rule): the high
+// parts are added with an error-free transformation, the error and the low parts in plain double.  One fp64 operation
+// on the dependent chain per addition instead of ~13 (an fp64 add has ~20 cycles of latency on B200 and these chains
+// run in ONE warp while the whole GPU waits); the pair is not renormalised -- dd_round adds the two parts once.  The
+// low part carries n * 2^-53 relative error of ITSELF, i.e. ~2^-99 of the largest partial sum: the rounded result is
+// still the correctly rounded exact sum unless that lies within ~1e-29 (relative) of a rounding boundary.
+__host__ __device__ __forceinline__ dd dd_acc(dd a, dd b) {
+    dd s = two_sum(a.hi, b.hi);
+    s.lo += a.lo + b.lo;
+    return s;
+}
 __host__ __device__ __forceinline__ dd dd_neg(dd a) { return dd{-a.hi, -a.lo}; }
 __host__ __device__ __forceinline__ dd dd_mul(dd a, dd b) {
     dd p = two_prod(a.hi, b.hi);

@@ -267,16 +267,24 @@ inline void compress_columns(HostSell& S, bool enable) {
 }
 
 
-// Validate the caller's CSR (A0) and return "" or the reason it is rejected.
-inline std::string validate_csr(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, const int32_t* col_idx,
-                                const double* val, const char* sense, const double* b, const double* c,
-                                const double* l, const double* u) {
+// Validate the caller's CSR (A0) and return "" or the reason it is rejected.  Two parts: validate_args looks at the
+// sizes and pointers only (what must hold before any array is read or copied); validate_entries scans the arrays
+// (uc_lp_create runs it on a helper thread while the arrays are being copied to the device, and waits for it before
+// the first kernel reads them).
+inline std::string validate_args(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, const int32_t* col_idx,
+                                 const double* val, const char* sense, const double* b, const double* c,
+                                 const double* l, const double* u) {
     if (m < 0 || n < 0 || nnz < 0) return "negative size";
     if (!row_ptr) return "row_ptr is NULL";
     if (m > 2000000000LL || n > 2000000000LL || nnz > 2000000000LL) return "size exceeds the int32 index range of the layout";
     if (row_ptr[0] != 0 || row_ptr[m] != nnz) return "row_ptr[0] != 0 or row_ptr[m] != nnz";
     if (nnz > 0 && (!col_idx || !val)) return "col_idx / val is NULL";
     if ((m > 0 && (!sense || !b)) || (n > 0 && (!c || !l || !u))) return "a vector argument is NULL";
+    return "";
+}
+inline std::string validate_entries(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, const int32_t* col_idx,
+                                    const double* val, const char* sense, const double* b, const double* c,
+                                    const double* l, const double* u) {
     for (int64_t i = 0; i < m; ++i)
         if (row_ptr[i + 1] < row_ptr[i] || row_ptr[i + 1] > nnz) return "row_ptr is not monotone";
     // rows are checked in parallel ranges, each with its own duplicate-detection stamps; the reported reason is
@@ -309,6 +317,12 @@ inline std::string validate_csr(int64_t m, int64_t n, int64_t nnz, const int64_t
         if (l[j] > u[j]) return "l > u";
     }
     return "";
+}
+inline std::string validate_csr(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, const int32_t* col_idx,
+                                const double* val, const char* sense, const double* b, const double* c,
+                                const double* l, const double* u) {
+    std::string why = validate_args(m, n, nnz, row_ptr, col_idx, val, sense, b, c, l, u);
+    return why.empty() ? validate_entries(m, n, nnz, row_ptr, col_idx, val, sense, b, c, l, u) : why;
 }
 
 // A1 in three pieces, so that the caller can overlap them (and the upload of K) on two threads:

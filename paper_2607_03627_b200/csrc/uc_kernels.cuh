@@ -17,6 +17,7 @@
 #include <stdint.h>
 #include <math.h>
 #include <stddef.h>
+#include <assert.h>
 #include "../../include/uc_pdhg.h"
 #include "uc_dd.cuh"
 #include "uc_format.hpp"
@@ -89,7 +90,17 @@ struct Sell {
     int grid;              // nlblk + nblk, at least 1
     const StepDesc* steps;  // [steps_per_warp][sched_warps] schedule of the persistent attempt kernels (uc_attempt.cuh)
     int steps_per_warp, sched_warps;
+    long long nslots, ncols;   // stored slots of the sliced part; length of the vector the column indices address
+    int cta_warps;             // consumer warps per CTA of the attempt kernel that runs this schedule (+ 1 long-row warp)
 };
+// -DUC_DEBUG_BOUNDS: every address the attempt pipelines derive from a step descriptor or a stored column index is
+// checked on the device (compute-sanitizer is not available on every GPU pool; this build is the substitute and is run
+// through the GPU parity tests once per change of the pipelines, profiles/).
+#ifdef UC_DEBUG_BOUNDS
+#define UC_BOUNDS_ASSERT(cond) assert(cond)
+#else
+#define UC_BOUNDS_ASSERT(cond) do { } while (0)
+#endif
 
 struct Vecs {
     long long n, m;
@@ -196,7 +207,7 @@ __device__ __forceinline__ void warp_sum_dd_n(dd (&v)[NV]) {
             dd t;
             t.hi = __shfl_xor_sync(0xffffffffu, v[q].hi, o);
             t.lo = __shfl_xor_sync(0xffffffffu, v[q].lo, o);
-            v[q] = dd_add(v[q], t);
+            v[q] = dd_acc(v[q], t);                         // cascaded: see uc_dd.cuh
         }
     }
 }

@@ -4,6 +4,7 @@
 #include <atomic>
 #include <chrono>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <exception>
 #include <limits>
@@ -16,6 +17,7 @@
 #include "uc_format.hpp"
 #include "uc_kernels.cuh"
 #include "uc_attempt.cuh"
+#include "uc_ingest.cuh"
 
 using namespace ucpdhg;
 
@@ -78,16 +80,30 @@ struct uc_lp {
     cudaEvent_t ev_t0 = nullptr, ev_t1 = nullptr;
     // source maps for uc_lp_get_scaled_values (only with keep_source_map)
     std::vector<int64_t> k_src, k_lsrc, kt_src, kt_lsrc;
-    // host permutations (for warm starts / hooks)
-    std::vector<int64_t> h_perm_r, h_perm_c;
 
     // every array gets one slice (32 elements) of zeroed slack: the bulk copies of the attempt kernels read
-    // whole 32-row segments, and the last slice of the sliced part may be ragged
-    std::mutex alloc_mutex;                // uc_lp_create uploads the two layouts from two threads
+    // whole 32-row segments, and the last slice of the sliced part may be ragged.  Zeroing is ordered on the handle's
+    // stream, like everything else uc_lp_create does on the device.  With an arena reserved (the fixed set of vectors:
+    // one cudaMalloc instead of ~25) arrays are carved out of it.
+    std::mutex alloc_mutex;                // the host-ingest path uploads the two layouts from two threads
+    char* arena = nullptr; size_t arena_cap = 0, arena_used = 0;
+    void reserve_arena(size_t bytes) {
+        void* p = nullptr;
+        cudaError_t e = cudaMalloc(&p, bytes);
+        if (e != cudaSuccess) throw CudaFail{e, "cudaMalloc"};
+        if (cudaMemsetAsync(p, 0, bytes, own_stream) != cudaSuccess) throw CudaFail{cudaGetLastError(), "cudaMemsetAsync"};
+        std::lock_guard<std::mutex> g(alloc_mutex);
+        allocs.push_back(p); device_bytes += bytes;
+        arena = (char*)p; arena_cap = bytes; arena_used = 0;
+    }
     template <class T>
     T* dalloc(size_t count) {
         void* p = nullptr;
-        size_t bytes = (count + 32) * sizeof(T);
+        size_t bytes = (((count + 32) * sizeof(T) + 255) / 256) * 256;
+        {
+            std::lock_guard<std::mutex> g(alloc_mutex);
+            if (arena && arena_used + bytes <= arena_cap) { p = arena + arena_used; arena_used += bytes; return (T*)p; }
+        }
         cudaError_t e = cudaMalloc(&p, bytes);
         if (e != cudaSuccess) throw CudaFail{e, "cudaMalloc"};
         {
@@ -95,13 +111,21 @@ struct uc_lp {
             allocs.push_back(p);
             device_bytes += bytes;
         }
-        if (cudaMemset(p, 0, bytes) != cudaSuccess) throw CudaFail{cudaGetLastError(), "cudaMemset"};
+        if (cudaMemsetAsync(p, 0, bytes, own_stream) != cudaSuccess) throw CudaFail{cudaGetLastError(), "cudaMemsetAsync"};
         return (T*)p;
+    }
+    void dfree(void* p) {
+        if (!p) return;
+        std::lock_guard<std::mutex> g(alloc_mutex);
+        for (auto& q : allocs) if (q == p) { cudaFree(p); q = nullptr; return; }
     }
     template <class T>
     T* upload(const std::vector<T>& h) {
         T* d = dalloc<T>(h.size());
-        if (!h.empty()) CK(cudaMemcpy(d, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice));
+        if (!h.empty()) {
+            CK(cudaMemcpyAsync(d, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice, own_stream));
+            CK(cudaStreamSynchronize(own_stream));           // the source is pageable host memory of the caller's frame
+        }
         return d;
     }
 };
@@ -134,9 +158,153 @@ Sell upload_sell(uc_lp* lp, const HostSell& H) {
     if (S.grid < 1) S.grid = 1;
     S.steps = lp->upload(H.steps);
     S.steps_per_warp = (int)H.steps_per_warp; S.sched_warps = (int)H.sched_warps;
+    S.nslots = slots;
     return S;
 }
 
+
+// ------------------------------------------------------------------------------------------ A1 on the device
+// Temporary device memory of uc_lp_create: one allocation, bump-allocated, released when create returns.
+struct TempArena {
+    char* base = nullptr; size_t cap = 0, used = 0;
+    ~TempArena() { if (base) cudaFree(base); }
+    void reserve(size_t bytes) { CK(cudaMalloc((void**)&base, bytes)); cap = bytes; }
+    template <class T> T* get(size_t count) {
+        const size_t bytes = ((count * sizeof(T) + 255) / 256 + 1) * 256;
+        if (used + bytes > cap) throw CudaFail{cudaErrorMemoryAllocation, "temporary arena of uc_lp_create"};
+        T* p = (T*)(base + used); used += bytes; return p;
+    }
+};
+struct DevCsr { long long* ptr = nullptr; int* col = nullptr; double* val = nullptr; };   // the caller's CSR on the device
+struct DevPerm { long long* perm = nullptr; long long* inv = nullptr; long long nshort = 0; };
+
+long long d2h_ll(const long long* d, cudaStream_t st) {
+    long long h = 0;
+    CK(cudaMemcpyAsync(&h, d, sizeof h, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    return h;
+}
+// new -> old permutation of N rows with lengths len (uc_format.hpp build_perm), its inverse, and the short-row count
+DevPerm device_perm(uc_lp* lp, TempArena& T, const int* len, long long N, int thr, long long window, cudaStream_t st) {
+    DevPerm P;
+    P.perm = lp->dalloc<long long>((size_t)N); P.inv = T.get<long long>((size_t)N + 1);
+    if (N == 0) return P;
+    int* flag = T.get<int>((size_t)N); int* rank = T.get<int>((size_t)N + 1);
+    k_ing_short_flag<<<ing_grid(N), kIngestBlock, 0, st>>>(len, N, thr, flag);
+    size_t bytes = 0;
+    CK(cub::DeviceScan::ExclusiveSum(nullptr, bytes, flag, rank, N, st));
+    void* tmp = T.get<char>(bytes);
+    CK(cub::DeviceScan::ExclusiveSum(tmp, bytes, flag, rank, N, st));
+    int h_rank = 0, h_flag = 0;
+    CK(cudaMemcpyAsync(&h_rank, rank + (N - 1), sizeof(int), cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(&h_flag, flag + (N - 1), sizeof(int), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    P.nshort = (long long)h_rank + h_flag;
+    unsigned long long *k0 = T.get<unsigned long long>((size_t)P.nshort + 1), *k1 = T.get<unsigned long long>((size_t)P.nshort + 1);
+    int *v0 = T.get<int>((size_t)P.nshort + 1), *v1 = T.get<int>((size_t)P.nshort + 1);
+    k_ing_perm_keys<<<ing_grid(N), kIngestBlock, 0, st>>>(len, rank, N, thr, window, P.nshort, k0, v0, P.perm);
+    if (P.nshort > 0) {
+        const unsigned long long maxkey = (unsigned long long)((P.nshort - 1) / window) * (unsigned long long)(thr + 1) + (unsigned long long)thr;
+        const int end_bit = bits_for(maxkey);
+        CK(cub::DeviceRadixSort::SortPairs(nullptr, bytes, k0, k1, v0, v1, P.nshort, 0, end_bit, st));
+        tmp = T.get<char>(bytes);
+        CK(cub::DeviceRadixSort::SortPairs(tmp, bytes, k0, k1, v0, v1, P.nshort, 0, end_bit, st));    // stable
+    }
+    k_ing_perm_finish<<<ing_grid(N), kIngestBlock, 0, st>>>(v1, P.nshort, N, P.perm, P.inv);
+    return P;
+}
+// One side (K or K'): slice pointers, sliced-ELL arrays, long tail, 16-bit offsets, schedule.  Returns the device
+// layout; fills the counters of the handle through the out parameters.
+struct SideStats { int64_t slots = 0, long_nnz = 0, narrow = 0; };
+Sell device_side(uc_lp* lp, TempArena& T, const FillSrc& S, const int* len, long long N, const DevPerm& P, const long long* inv_other,
+                 bool compress, bool want_src, int ctas, int warps_per_cta, cudaStream_t st, SideStats& stats,
+                 std::vector<int64_t>* h_src, std::vector<int64_t>* h_lsrc) {
+    Sell A{};
+    const long long nshort = P.nshort, nlong = N - nshort, nslices = (nshort + 31) / 32;
+    // slice pointers
+    long long* slots = T.get<long long>((size_t)nslices + 1);
+    long long* sp = lp->dalloc<long long>((size_t)nslices + 1);
+    if (nslices) k_ing_slice_width<<<ing_grid(nslices), kIngestBlock, 0, st>>>(len, P.perm, nshort, nslices, slots);
+    size_t bytes = 0; void* tmp = nullptr;
+    if (nslices) {
+        CK(cub::DeviceScan::ExclusiveSum(nullptr, bytes, slots, sp, nslices, st));
+        tmp = T.get<char>(bytes);
+        CK(cub::DeviceScan::ExclusiveSum(tmp, bytes, slots, sp, nslices, st));
+    }
+    k_ing_close_scan<<<1, 32, 0, st>>>(sp, slots, nslices);
+    // long tail pointers
+    long long* llen = T.get<long long>((size_t)nlong + 1);
+    long long* lptr = lp->dalloc<long long>((size_t)nlong + 1);
+    if (nlong) {
+        k_ing_long_len<<<ing_grid(nlong), kIngestBlock, 0, st>>>(len, P.perm, nshort, nlong, llen);
+        CK(cub::DeviceScan::ExclusiveSum(nullptr, bytes, llen, lptr, nlong, st));
+        tmp = T.get<char>(bytes);
+        CK(cub::DeviceScan::ExclusiveSum(tmp, bytes, llen, lptr, nlong, st));
+    }
+    k_ing_close_scan<<<1, 32, 0, st>>>(lptr, llen, nlong);
+    const long long nslots = d2h_ll(sp + nslices, st), lnnz = d2h_ll(lptr + nlong, st);
+    if (nslots >= (1LL << 31)) throw std::bad_alloc();              // step descriptors address entries / 32 in 26 bits
+    stats.slots = nslots; stats.long_nnz = lnnz;
+    // arrays (zeroed by dalloc: padding slots are (col 0, val 0.0))
+    int* col = lp->dalloc<int>((size_t)nslots);
+    double* val = lp->dalloc<double>((size_t)nslots);
+    int* lcol = lp->dalloc<int>((size_t)lnnz);
+    double* lval = lp->dalloc<double>((size_t)lnnz);
+    long long *src = nullptr, *lsrc = nullptr;
+    if (want_src) {
+        src = T.get<long long>((size_t)nslots + 1); lsrc = T.get<long long>((size_t)lnnz + 1);
+        CK(cudaMemsetAsync(src, 0xff, sizeof(long long) * (size_t)nslots, st));             // -1 = padding
+    }
+    if (nshort) k_ing_fill_sell<<<ing_grid(nshort), kIngestBlock, 0, st>>>(S, P.perm, inv_other, nshort, sp, col, val, src);
+    if (nlong) k_ing_fill_long<<<ing_grid(nlong * 32), kIngestBlock, 0, st>>>(S, P.perm, inv_other, nshort, nlong, lptr, lcol, lval, lsrc);
+    // 16-bit offsets
+    int* cbase = lp->dalloc<int>((size_t)nslices);
+    long long* narrow_of = T.get<long long>((size_t)nslices + 1);
+    long long* narrow_sum = T.get<long long>(1);
+    unsigned short* col16 = nullptr;
+    long long narrow = 0;
+    if (nslices) {
+        k_ing_slice_base<<<ing_grid(nslices * 32), kIngestBlock, 0, st>>>(len, P.perm, nshort, nslices, sp, col, compress ? 1 : 0, cbase, narrow_of);
+        CK(cub::DeviceReduce::Sum(nullptr, bytes, narrow_of, narrow_sum, nslices, st));
+        tmp = T.get<char>(bytes);
+        CK(cub::DeviceReduce::Sum(tmp, bytes, narrow_of, narrow_sum, nslices, st));
+        narrow = d2h_ll(narrow_sum, st);
+        if (narrow > 0) {
+            col16 = lp->dalloc<unsigned short>((size_t)nslots);
+            k_ing_col16<<<ing_grid(nshort), kIngestBlock, 0, st>>>(len, P.perm, nshort, nslices, sp, col, cbase, col16);
+        }
+    }
+    stats.narrow = narrow;
+    // schedule on the host from the slice bases and the per-slice index bases
+    HostSell H;
+    H.nslices = nslices; H.nshort = nshort; H.nlong = nlong; H.nrows = N;
+    H.slice_ptr.assign((size_t)nslices + 1, 0); H.cbase.assign((size_t)nslices, -1);
+    CK(cudaMemcpyAsync(H.slice_ptr.data(), sp, sizeof(long long) * (size_t)(nslices + 1), cudaMemcpyDeviceToHost, st));
+    if (nslices) CK(cudaMemcpyAsync(H.cbase.data(), cbase, sizeof(int) * (size_t)nslices, cudaMemcpyDeviceToHost, st));
+    if (want_src) {
+        h_src->resize((size_t)nslots); h_lsrc->resize((size_t)lnnz);
+        if (nslots) CK(cudaMemcpyAsync(h_src->data(), src, sizeof(long long) * (size_t)nslots, cudaMemcpyDeviceToHost, st));
+        if (lnnz) CK(cudaMemcpyAsync(h_lsrc->data(), lsrc, sizeof(long long) * (size_t)lnnz, cudaMemcpyDeviceToHost, st));
+    }
+    CK(cudaStreamSynchronize(st));
+    build_schedule(H, ctas, warps_per_cta);
+    A.sp = sp; A.col = col; A.col16 = col16; A.cbase = cbase; A.val = val;
+    A.nshort = nshort; A.nslices = (int)nslices; A.nblk = cdiv(nslices, kWarps);
+    A.lp = lptr; A.lcol = lcol; A.lval = lval; A.nlong = (int)nlong; A.nlblk = cdiv(nlong, kWarps);
+    A.grid = std::max(1, A.nlblk + A.nblk);
+    A.steps = lp->upload(H.steps);
+    A.steps_per_warp = (int)H.steps_per_warp; A.sched_warps = (int)H.sched_warps;
+    A.nslots = nslots;
+    if (narrow == nslots && nslots > 0) { lp->dfree(col); A.col = nullptr; }            // every slice is narrow: the 32-bit copy is not kept
+    return A;
+}
+
+// two-stage reduction of a device array into one device double (op 0: sum of squares, 1: max |v|); stream-ordered, no sync
+void reduce_to_dev(const double* v, long long count, int op, dd* part, double* out_dev, cudaStream_t st) {
+    int blocks = count > 0 ? (int)std::min<long long>(1024, (count + kBlock - 1) / kBlock) : 1;
+    k_reduce<<<blocks, kBlock, 0, st>>>(v, count, op, part);
+    k_reduce_final<<<1, 32, 0, st>>>(part, blocks, op, out_dev);
+}
 // two-stage reduction of a device array to one host double (op 0: sum of squares, 1: max |v|)
 double reduce_to_host(uc_lp* lp, const double* v, long long count, int op, dd* part, double* out_dev, cudaStream_t st) {
     int blocks = count > 0 ? std::min<long long>(1024, (count + kBlock - 1) / kBlock) : 1;
@@ -233,8 +401,8 @@ constexpr size_t kAttemptSmemBytes = UC_SMEM_REQUEST;
 constexpr size_t kAttemptSmemBytes = kPrimalSmemBytes > kDualSmemBytes ? kPrimalSmemBytes : kDualSmemBytes;
 #endif
 static_assert(kAttemptSmemBytes >= kPrimalSmemBytes && kAttemptSmemBytes >= kDualSmemBytes, "shared memory request");
-void launch_primal(uc_lp* lp, cudaStream_t st) { launch_pdl(k_primal, lp->V.gridPA, kPrimalThreads, kAttemptSmemBytes, st, lp->KT, lp->V, lp->ctl); }
-void launch_dual(uc_lp* lp, cudaStream_t st) { launch_pdl(k_dual, lp->V.gridPB, kDualThreads, kAttemptSmemBytes, st, lp->K, lp->V, lp->ctl); }
+void launch_primal(uc_lp* lp, cudaStream_t st) { launch_pdl(k_primal, lp->V.gridPA, (lp->KT.cta_warps + 1) * 32, kAttemptSmemBytes, st, lp->KT, lp->V, lp->ctl); }
+void launch_dual(uc_lp* lp, cudaStream_t st) { launch_pdl(k_dual, lp->V.gridPB, (lp->K.cta_warps + 1) * 32, kAttemptSmemBytes, st, lp->K, lp->V, lp->ctl); }
 void launch_attempt(uc_lp* lp, cudaStream_t st) { launch_primal(lp, st); launch_dual(lp, st); }
 void launch_kkt(uc_lp* lp, cudaStream_t st, int mode) {
     const int flush = mode == kModeCheck;        // the periodic check also applies the pending average term (R6)
@@ -291,7 +459,7 @@ void destroy_impl(uc_lp* lp) {
     for (auto& e : lp->ev) if (e) cudaEventDestroy(e);
     if (lp->ev_t0) cudaEventDestroy(lp->ev_t0);
     if (lp->ev_t1) cudaEventDestroy(lp->ev_t1);
-    for (void* p : lp->allocs) cudaFree(p);
+    for (void* p : lp->allocs) if (p) cudaFree(p);
     if (lp->powtab) cudaFree(lp->powtab);
     if (lp->h_status) cudaFreeHost(lp->h_status);
     if (lp->h_stop) cudaFreeHost(lp->h_stop);
@@ -481,7 +649,7 @@ double uc_host_exp_rounded(double x) { return exp_rounded(x); }
 void uc_lp_default_options(uc_lp_options* o) {
     if (!o) return;
     o->device = -1; o->ruiz_iters = 10; o->pc_alpha = 1.0; o->sell_window = 4096; o->long_row_threshold = 32;
-    o->keep_source_map = 0; o->index_compression = 1;
+    o->keep_source_map = 0; o->index_compression = 1; o->host_ingest = 0;
 }
 
 void uc_pdhg_default_params(uc_pdhg_params* p) {
@@ -504,15 +672,29 @@ int uc_lp_create(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, cons
     if (opt_in) opt = *opt_in;
     if (opt.ruiz_iters < 0 || opt.pc_alpha < 0.0 || opt.pc_alpha > 2.0 || opt.sell_window < 32 || opt.long_row_threshold < 1)
         return fail(UC_ERR_INVALID, "bad uc_lp_options");
-    std::string why = validate_csr(m, n, nnz, row_ptr, col_idx, val, sense, b, c, l, u);
+    const bool tim = std::getenv("UC_CREATE_TIMING") != nullptr;
+    double tph = now_s();
+    auto phase = [&](const char* what) { if (tim) { double t = now_s(); std::fprintf(stderr, "  create: %-28s %7.2f ms\n", what, (t - tph) * 1e3); tph = t; } };
+    std::string why = validate_args(m, n, nnz, row_ptr, col_idx, val, sense, b, c, l, u);
     if (!why.empty()) return fail(UC_ERR_INVALID, why);
+    // A0: the arrays are scanned on a helper thread while this thread copies them to the device; no kernel reads them
+    // before the verdict is in (join_validation), and bad input is still rejected when there is no device at all
+    std::string why_entries;
+    std::thread validator([&] {
+        try { why_entries = validate_entries(m, n, nnz, row_ptr, col_idx, val, sense, b, c, l, u); }
+        catch (...) { why_entries = "host allocation failed during validation"; }
+    });
+    bool validated = false;
+    auto join_validation = [&]() { if (!validated) { validator.join(); validated = true; } return why_entries.empty(); };
 
     int ndev = 0;
-    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        if (!join_validation()) return fail(UC_ERR_INVALID, why_entries);
         return fail(UC_ERR_CUDA, "no CUDA device: this library has no CPU path");
+    }
     int dev = opt.device;
-    if (dev < 0) { if (cudaGetDevice(&dev) != cudaSuccess) return fail(UC_ERR_CUDA, "cudaGetDevice failed"); }
-    if (dev >= ndev) return fail(UC_ERR_INVALID, "device ordinal out of range");
+    if (dev < 0 && cudaGetDevice(&dev) != cudaSuccess) { join_validation(); return fail(UC_ERR_CUDA, "cudaGetDevice failed"); }
+    if (dev >= ndev) { join_validation(); return fail(UC_ERR_INVALID, "device ordinal out of range"); }
 
     uc_lp* lp = nullptr;
     try {
@@ -524,21 +706,110 @@ int uc_lp_create(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, cons
         CK(cudaEventCreate(&lp->ev_t0)); CK(cudaEventCreate(&lp->ev_t1));
         cudaStream_t st = lp->own_stream;
 
-        // A0 / A1: layouts (host), upload.  The K side (layout, schedule, upload) runs on a helper thread while this
-        // thread transposes and builds the K' side.
+        const bool want_src = opt.keep_source_map != 0;
+        int sms = 0, warpsPA = kPrimalWarps, warpsPB = kDualWarps;
+        CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+        // persistent grids of the attempt kernels: kCtasPerSm CTAs per SM, never more CTAs than work, and no more
+        // consumer warps per CTA than the slices need (at least kMinWarps, at most the compiled maximum)
+        auto attempt_shape = [&](int64_t nshort, int64_t nlong, int max_warps, int& grid, int& warps) {
+            const int64_t cap = (int64_t)kCtasPerSm * std::max(sms, 1), slices = (nshort + 31) / 32;
+            warps = (int)std::max<int64_t>(std::min<int64_t>(kMinWarps, max_warps), std::min<int64_t>(max_warps, (slices + cap - 1) / cap));
+            grid = (int)std::max<int64_t>(1, std::min<int64_t>(cap, std::max<int64_t>((slices + warps - 1) / warps, nlong)));
+        };
+        auto attempt_grids = [&](int64_t nshort_r, int64_t nshort_c, int& gridPA, int& gridPB) {
+            attempt_shape(nshort_c, n - nshort_c, kPrimalWarps, gridPA, warpsPA);
+            attempt_shape(nshort_r, m - nshort_r, kDualWarps, gridPB, warpsPB);
+        };
+        int gridPA = 1, gridPB = 1;
+        TempArena T;                                               // released when create returns
+        // the data vectors (original order, temporary) go up on a helper thread with its own stream, next to the CSR
+        TempArena TV;
+        TV.reserve((size_t)8 * (size_t)(m + 3 * n) + (size_t)m + 8 * 512 + sizeof(dd) * 1024 + 4096);
+        double* db = TV.get<double>((size_t)m + 1); double* dc = TV.get<double>((size_t)n + 1);
+        double* dl = TV.get<double>((size_t)n + 1); double* du = TV.get<double>((size_t)n + 1);
+        char* dsense = TV.get<char>((size_t)m + 1);
+        dd* part = TV.get<dd>(1024); double* scal = TV.get<double>(8);
+        cudaError_t vec_err = cudaSuccess;
+        std::thread vec_up([&] {
+            cudaSetDevice(dev);
+            cudaStream_t s2 = nullptr;
+            vec_err = cudaStreamCreateWithFlags(&s2, cudaStreamNonBlocking);
+            auto up = [&](void* d, const void* h, size_t bytes) { if (vec_err == cudaSuccess && bytes) vec_err = cudaMemcpyAsync(d, h, bytes, cudaMemcpyHostToDevice, s2); };
+            up(db, b, sizeof(double) * (size_t)m); up(dc, c, sizeof(double) * (size_t)n);
+            up(dl, l, sizeof(double) * (size_t)n); up(du, u, sizeof(double) * (size_t)n); up(dsense, sense, (size_t)m);
+            if (vec_err == cudaSuccess) vec_err = cudaStreamSynchronize(s2);
+            if (s2) cudaStreamDestroy(s2);
+        });
+        struct Joiner { std::thread& t; ~Joiner() { if (t.joinable()) t.join(); } } vec_joiner{vec_up};
+        phase("stream/events");
+        if (!opt.host_ingest) {
+            // ---- A1 on the device (uc_ingest.cuh): one copy of the caller's CSR, then kernels
+            const size_t src_bytes = want_src ? 16 * ((size_t)nnz + 32 * (size_t)(m + n) / 32 + 1024) * 3 : 0;
+            T.reserve((size_t)(8 * (m + 1) + 44 * nnz + 28 * n + 4 * m + 44 * (m + n)) + ((size_t)(m + n) / 32 + 2) * 40 +
+                      src_bytes + 256 * 64 + ((size_t)64 << 20));
+            long long* d_ptr = T.get<long long>((size_t)m + 1);
+            int* d_col = T.get<int>((size_t)nnz + 1);
+            double* d_val = T.get<double>((size_t)nnz + 1);
+            CK(cudaMemcpyAsync(d_ptr, row_ptr, sizeof(long long) * (size_t)(m + 1), cudaMemcpyHostToDevice, st));
+            if (nnz) {
+                CK(cudaMemcpyAsync(d_col, col_idx, sizeof(int) * (size_t)nnz, cudaMemcpyHostToDevice, st));
+                CK(cudaMemcpyAsync(d_val, val, sizeof(double) * (size_t)nnz, cudaMemcpyHostToDevice, st));
+            }
+            phase("H2D of the CSR");
+            if (!join_validation()) { destroy_impl(lp); return fail(UC_ERR_INVALID, why_entries); }
+            phase("validation verdict");
+            int* lenr = T.get<int>((size_t)m + 1); int* lenc = T.get<int>((size_t)n + 1);
+            int* rowid = T.get<int>((size_t)nnz + 1);
+            CK(cudaMemsetAsync(lenc, 0, sizeof(int) * (size_t)(n + 1), st));
+            if (m) k_ing_row_len<<<ing_grid(m), kIngestBlock, 0, st>>>(d_ptr, m, lenr);
+            if (nnz) {
+                k_ing_col_count<<<ing_grid(nnz), kIngestBlock, 0, st>>>(d_col, nnz, lenc);
+                k_ing_row_ids<<<ing_grid(nnz), kIngestBlock, 0, st>>>(d_ptr, m, nnz, rowid);
+            }
+            DevPerm Pr = device_perm(lp, T, lenr, m, opt.long_row_threshold, opt.sell_window, st);
+            DevPerm Pc = device_perm(lp, T, lenc, n, opt.long_row_threshold, opt.sell_window, st);
+            attempt_grids(Pr.nshort, Pc.nshort, gridPA, gridPB);
+            // explicit transpose: column pointers + the entries in (column, caller's row) order
+            long long* tptr = T.get<long long>((size_t)n + 2);
+            int* order = T.get<int>((size_t)nnz + 1);
+            {
+                long long* wide = T.get<long long>((size_t)n + 1);
+                size_t bytes = 0; void* tmp = nullptr;
+                if (n) {
+                    k_ing_widen<<<ing_grid(n), kIngestBlock, 0, st>>>(lenc, wide, n);
+                    CK(cub::DeviceScan::ExclusiveSum(nullptr, bytes, wide, tptr, n, st));
+                    tmp = T.get<char>(bytes);
+                    CK(cub::DeviceScan::ExclusiveSum(tmp, bytes, wide, tptr, n, st));
+                }
+                k_ing_close_scan<<<1, 32, 0, st>>>(tptr, wide, n);
+                if (nnz) {
+                    unsigned* k0 = reinterpret_cast<unsigned*>(d_col);                     // column indices are >= 0
+                    unsigned* k1 = T.get<unsigned>((size_t)nnz + 1);
+                    int* v0 = T.get<int>((size_t)nnz + 1);
+                    k_ing_iota<<<ing_grid(nnz), kIngestBlock, 0, st>>>(v0, nnz);
+                    const int end_bit = bits_for((unsigned long long)std::max<int64_t>(n - 1, 1));
+                    CK(cub::DeviceRadixSort::SortPairs(nullptr, bytes, k0, k1, v0, order, nnz, 0, end_bit, st));
+                    tmp = T.get<char>(bytes);
+                    CK(cub::DeviceRadixSort::SortPairs(tmp, bytes, k0, k1, v0, order, nnz, 0, end_bit, st));   // stable: rows ascend inside a column
+                }
+            }
+            SideStats sk, skt;
+            lp->K = device_side(lp, T, FillSrc{d_ptr, nullptr, d_col, d_val}, lenr, m, Pr, Pc.inv, opt.index_compression != 0, want_src,
+                                gridPB, warpsPB, st, sk, &lp->k_src, &lp->k_lsrc);
+            lp->KT = device_side(lp, T, FillSrc{tptr, order, rowid, d_val}, lenc, n, Pc, Pr.inv, opt.index_compression != 0, want_src,
+                                 gridPA, warpsPA, st, skt, &lp->kt_src, &lp->kt_lsrc);
+            lp->k_slots = sk.slots; lp->kt_slots = skt.slots; lp->k_long_nnz = sk.long_nnz; lp->kt_long_nnz = skt.long_nnz;
+            lp->k_narrow = sk.narrow; lp->kt_narrow = skt.narrow;
+            lp->perm_r = Pr.perm; lp->perm_c = Pc.perm;
+            phase("device ingest");
+        } else {
+        // ---- A1 on the host (uc_format.hpp; the checker's builders): layouts on up to 8 threads, then uploaded.  The K
+        // side (layout, schedule, upload) runs on a helper thread while this thread transposes and builds the K' side.
+        if (!join_validation()) { destroy_impl(lp); return fail(UC_ERR_INVALID, why_entries); }
         HostProblem P;
         build_perms(m, n, nnz, row_ptr, col_idx, opt.sell_window, opt.long_row_threshold, P);
-        int gridPA = 1, gridPB = 1;
-        {   // persistent grids of the attempt kernels: kCtasPerSm CTAs per SM, never more CTAs than work; the static
-            // schedule gives every slice to the consumer warp with the least work so far
-            int sms = 0;
-            CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-            const int cap = kCtasPerSm * std::max(sms, 1);
-            const int64_t sl_kt = (P.nshort_c + 31) / 32, sl_k = (P.nshort_r + 31) / 32;
-            gridPA = (int)std::max<int64_t>(1, std::min<int64_t>(cap, std::max<int64_t>((sl_kt + kPrimalWarps - 1) / kPrimalWarps, n - P.nshort_c)));
-            gridPB = (int)std::max<int64_t>(1, std::min<int64_t>(cap, std::max<int64_t>((sl_k + kDualWarps - 1) / kDualWarps, m - P.nshort_r)));
-        }
-        const bool want_src = opt.keep_source_map != 0;
+        phase("perms");
+        attempt_grids(P.nshort_r, P.nshort_c, gridPA, gridPB);
         std::exception_ptr k_side_error;
         std::thread k_side([&] {
             try {
@@ -546,29 +817,36 @@ int uc_lp_create(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, cons
                 build_K(row_ptr, col_idx, val, want_src, P);
                 if (P.K.col.size() >= (size_t)1 << 31) throw std::bad_alloc();   // step descriptors address entries / 32 in 26 bits
                 compress_columns(P.K, opt.index_compression != 0);
-                build_schedule(P.K, gridPB, kDualWarps);
+                build_schedule(P.K, gridPB, warpsPB);
                 lp->K = upload_sell(lp, P.K);
             } catch (...) { k_side_error = std::current_exception(); }
         });
         try {
             build_KT(row_ptr, col_idx, val, want_src, P);
+            phase("build_KT");
             if (P.KT.col.size() >= (size_t)1 << 31) throw std::bad_alloc();
             compress_columns(P.KT, opt.index_compression != 0);
-            build_schedule(P.KT, gridPA, kPrimalWarps);
+            phase("compress KT");
+            build_schedule(P.KT, gridPA, warpsPA);
+            phase("schedule KT");
             lp->KT = upload_sell(lp, P.KT);
+            phase("upload KT");
         } catch (...) { k_side.join(); throw; }
         k_side.join();
+        phase("join K side");
         if (k_side_error) std::rethrow_exception(k_side_error);
         lp->k_slots = (int64_t)P.K.col.size(); lp->kt_slots = (int64_t)P.KT.col.size();
         lp->k_long_nnz = (int64_t)P.K.lcol.size(); lp->kt_long_nnz = (int64_t)P.KT.lcol.size();
         lp->k_narrow = P.K.narrow_slots; lp->kt_narrow = P.KT.narrow_slots;
         lp->perm_r = (long long*)lp->upload(P.perm_r);
         lp->perm_c = (long long*)lp->upload(P.perm_c);
-        lp->h_perm_r = P.perm_r; lp->h_perm_c = P.perm_c;
         if (opt.keep_source_map) { lp->k_src = std::move(P.K.src); lp->k_lsrc = std::move(P.K.lsrc); lp->kt_src = std::move(P.KT.src); lp->kt_lsrc = std::move(P.KT.lsrc); }
 
+        }
+        lp->K.ncols = n; lp->KT.ncols = m; lp->K.cta_warps = warpsPB; lp->KT.cta_warps = warpsPA;
         Vecs& V = lp->V;
         V.n = n; V.m = m;
+        lp->reserve_arena((size_t)(11 * 8 + 16) * (size_t)(n + 64) + (size_t)(7 * 8 + 1) * (size_t)(m + 64) + ((size_t)1 << 20));
         for (int i = 0; i < 2; ++i) { V.x[i] = lp->dalloc<double>((size_t)n); V.y[i] = lp->dalloc<double>((size_t)m); }
         V.xg = lp->dalloc<double2>((size_t)n);
         V.xsum = lp->dalloc<double>((size_t)n); V.ysum = lp->dalloc<double>((size_t)m);
@@ -593,54 +871,58 @@ int uc_lp_create(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, cons
         V.partP = lp->dalloc<dd>((size_t)6 * V.gridB);
         V.partR = lp->dalloc<dd>((size_t)2 * V.gridR);
         lp->ctl = lp->dalloc<Ctrl>(1);
-        CK(cudaMemset(lp->ctl, 0, sizeof(Ctrl)));
+        CK(cudaMemsetAsync(lp->ctl, 0, sizeof(Ctrl), st));
         CK(cudaHostAlloc((void**)&lp->h_status, sizeof(HostStatus), cudaHostAllocMapped));
         CK(cudaHostAlloc((void**)&lp->h_stop, sizeof(int), cudaHostAllocMapped));
         std::memset(lp->h_status, 0, sizeof(HostStatus)); *lp->h_stop = 0;
         CK(cudaHostGetDevicePointer((void**)&lp->d_status, lp->h_status, 0));
         CK(cudaHostGetDevicePointer((void**)&lp->d_stop, lp->h_stop, 0));
 
-        // original-order copies of the data vectors (temporary)
-        double *db = nullptr, *dc = nullptr, *dl = nullptr, *du = nullptr; char* dsense = nullptr;
-        auto tmp_up = [&](const void* h, size_t bytes) { void* p = nullptr; CK(cudaMalloc(&p, bytes ? bytes : 1)); if (bytes) CK(cudaMemcpy(p, h, bytes, cudaMemcpyHostToDevice)); return p; };
-        db = (double*)tmp_up(b, sizeof(double) * (size_t)m); dc = (double*)tmp_up(c, sizeof(double) * (size_t)n);
-        dl = (double*)tmp_up(l, sizeof(double) * (size_t)n); du = (double*)tmp_up(u, sizeof(double) * (size_t)n);
-        dsense = (char*)tmp_up(sense, (size_t)m);
-        dd* part = nullptr; double* scal = nullptr;
-        CK(cudaMalloc((void**)&part, sizeof(dd) * 1024)); CK(cudaMalloc((void**)&scal, sizeof(double)));
-
-        // unscaled norms for R9 (before anything is scaled)
-        lp->norm_b = std::sqrt(reduce_to_host(lp, db, m, 0, part, scal, st));
-        lp->norm_c = std::sqrt(reduce_to_host(lp, dc, n, 0, part, scal, st));
-
-        // A2, A3: preconditioning;  A4: scaled data and the initial scalars of R2
+        vec_up.join();
+        if (vec_err != cudaSuccess) throw CudaFail{vec_err, "upload of b, c, l, u, sense"};
+        phase("vectors alloc + upload");
+        // unscaled norms for R9 (before anything is scaled); A2, A3: preconditioning; A4: scaled data and the initial
+        // scalars of R2.  The six scalars come back in ONE copy.
+        reduce_to_dev(db, m, 0, part, scal + 0, st);
+        reduce_to_dev(dc, n, 0, part, scal + 1, st);
         CK(cudaEventRecord(lp->ev_t0, st));
         precondition(lp, st);
         k_scale_problem<<<V.gridR, kBlock, 0, st>>>(n, m, db, dc, dl, du, dsense, lp->perm_c, lp->perm_r, lp->Dr, lp->Dc,
                                                     lp->qs, lp->cs, lp->ls, lp->us, lp->isG);
         CK(cudaGetLastError());
-        double kmax = reduce_to_host(lp, lp->K.val, lp->k_slots, 1, part, scal, st);
-        kmax = std::max(kmax, reduce_to_host(lp, lp->K.lval, lp->k_long_nnz, 1, part, scal, st));
-        const double ncs = std::sqrt(reduce_to_host(lp, lp->cs, n, 0, part, scal, st));
-        const double nqs = std::sqrt(reduce_to_host(lp, lp->qs, m, 0, part, scal, st));
+        reduce_to_dev(lp->K.val, lp->k_slots, 1, part, scal + 2, st);
+        reduce_to_dev(lp->K.lval, lp->k_long_nnz, 1, part, scal + 3, st);
+        reduce_to_dev(lp->cs, n, 0, part, scal + 4, st);
+        reduce_to_dev(lp->qs, m, 0, part, scal + 5, st);
         CK(cudaEventRecord(lp->ev_t1, st));
+        double hs[6];
+        CK(cudaMemcpyAsync(hs, scal, sizeof hs, cudaMemcpyDeviceToHost, st));
         CK(cudaStreamSynchronize(st));
         float ms = 0.f; CK(cudaEventElapsedTime(&ms, lp->ev_t0, lp->ev_t1));
         lp->precondition_seconds = ms * 1e-3;
+        lp->norm_b = std::sqrt(hs[0]); lp->norm_c = std::sqrt(hs[1]);
+        const double kmax = std::max(hs[2], hs[3]), ncs = std::sqrt(hs[4]), nqs = std::sqrt(hs[5]);
         lp->eta0 = kmax > 0.0 ? 1.0 / kmax : 1.0;
         lp->omega0 = (ncs > 1e-10 && nqs > 1e-10) ? ncs / nqs : 1.0;
         lp->norm_qs = nqs;
-        cudaFree(db); cudaFree(dc); cudaFree(dl); cudaFree(du); cudaFree(dsense); cudaFree(part); cudaFree(scal);
+        phase("precondition + scalars");
         lp->create_seconds = now_s() - t_create;
     } catch (const CudaFail& f) {
         std::string msg = std::string(f.what) + ": " + cudaGetErrorString(f.e);
         int code = (f.e == cudaErrorMemoryAllocation) ? UC_ERR_NOMEM : UC_ERR_CUDA;
+        join_validation();
         destroy_impl(lp);
         return fail(code, msg);
     } catch (const std::bad_alloc&) {
+        join_validation();
         destroy_impl(lp);
         return fail(UC_ERR_NOMEM, "host allocation failed");
+    } catch (const std::exception& e) {                       // std::system_error of a helper thread, std::length_error, ...
+        join_validation();
+        destroy_impl(lp);
+        return fail(UC_ERR_NOMEM, std::string("uc_lp_create: ") + e.what());
     }
+    join_validation();
     *out = lp;
     return UC_OK;
 }
@@ -833,6 +1115,8 @@ static int solve_impl(uc_lp* lp, const uc_pdhg_params* pin, double* x_out, doubl
         res->kernel_launches = launches;
     } catch (const CudaFail& f) {
         rc = fail((f.e == cudaErrorMemoryAllocation) ? UC_ERR_NOMEM : UC_ERR_CUDA, std::string(f.what) + ": " + cudaGetErrorString(f.e));
+    } catch (const std::exception& e) {                        // nothing may unwind through the C ABI
+        rc = fail(UC_ERR_NOMEM, std::string("uc_pdhg_solve: ") + e.what());
     }
     if (tx0) cudaFree(tx0);
     if (ty0) cudaFree(ty0);
@@ -987,6 +1271,68 @@ int uc_lp_get_info(const uc_lp* lp, uc_lp_info* info) {
     return UC_OK;
 }
 
+// Test hook for A1: rebuild the permutations, both layouts and both schedules with the HOST builders (uc_format.hpp, the
+// code uc_host_layout_selftest checks against the caller's CSR) and compare them bit for bit with what the handle holds
+// on the device.  The matrix values are compared only if the handle was created without preconditioning (ruiz_iters = 0,
+// pc_alpha = 0), since uc_lp_create scales them in place.
+int uc_lp_compare_layout(uc_lp* lp, int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, const int32_t* col_idx, const double* val) {
+    if (!lp || !row_ptr || m != lp->m || n != lp->n || nnz != lp->nnz) return fail(UC_ERR_INVALID, "bad argument");
+    try {
+        DeviceGuard guard(lp->device);
+        HostProblem P;
+        build_perms(m, n, nnz, row_ptr, col_idx, lp->opt.sell_window, lp->opt.long_row_threshold, P);
+        build_K(row_ptr, col_idx, val, false, P);
+        build_KT(row_ptr, col_idx, val, false, P);
+        compress_columns(P.K, lp->opt.index_compression != 0);
+        compress_columns(P.KT, lp->opt.index_compression != 0);
+        build_schedule(P.K, lp->V.gridPB, lp->K.cta_warps);
+        build_schedule(P.KT, lp->V.gridPA, lp->KT.cta_warps);
+        const bool scaled = lp->opt.ruiz_iters > 0 || lp->opt.pc_alpha > 0.0;
+        std::string why;
+        auto same = [&](const char* what, const void* dev, const void* host, size_t bytes) {
+            if (!why.empty() || bytes == 0) return;
+            if (!dev) { why = std::string(what) + ": missing on the device"; return; }
+            std::vector<char> t(bytes);
+            CK(cudaMemcpy(t.data(), dev, bytes, cudaMemcpyDeviceToHost));
+            if (std::memcmp(t.data(), host, bytes) != 0) {
+                size_t k = 0; while (k < bytes && t[k] == ((const char*)host)[k]) ++k;
+                why = std::string(what) + ": differs at byte " + std::to_string(k);
+            }
+        };
+        same("row permutation", lp->perm_r, P.perm_r.data(), sizeof(int64_t) * (size_t)m);
+        same("column permutation", lp->perm_c, P.perm_c.data(), sizeof(int64_t) * (size_t)n);
+        auto side = [&](const char* name, const Sell& D, const HostSell& H) {
+            const std::string nm(name);
+            if (!why.empty()) return;
+            if (D.nshort != H.nshort || D.nslices != H.nslices || D.nlong != H.nlong) { why = nm + ": counts"; return; }
+            if (D.steps_per_warp != H.steps_per_warp || D.sched_warps != H.sched_warps) { why = nm + ": schedule shape"; return; }
+            const size_t slots = H.col.size();
+            same((nm + " slice pointers").c_str(), D.sp, H.slice_ptr.data(), sizeof(int64_t) * H.slice_ptr.size());
+            same((nm + " slice index bases").c_str(), D.cbase, H.cbase.data(), sizeof(int32_t) * H.cbase.size());
+            if ((size_t)H.narrow_slots < slots) same((nm + " 32-bit column indices").c_str(), D.col, H.col.data(), sizeof(int32_t) * slots);
+            else if (D.col && slots) why = nm + ": 32-bit column indices kept although every slice is narrow";
+            if (H.narrow_slots > 0) same((nm + " 16-bit column offsets").c_str(), D.col16, H.col16.data(), sizeof(uint16_t) * slots);
+            else if (D.col16) why = nm + ": 16-bit offsets present although no slice is narrow";
+            if (!scaled) same((nm + " values").c_str(), D.val, H.val.data(), sizeof(double) * slots);
+            same((nm + " long-row pointers").c_str(), D.lp, H.lptr.data(), sizeof(int64_t) * H.lptr.size());
+            same((nm + " long-row columns").c_str(), D.lcol, H.lcol.data(), sizeof(int32_t) * H.lcol.size());
+            if (!scaled) same((nm + " long-row values").c_str(), D.lval, H.lval.data(), sizeof(double) * H.lval.size());
+            same((nm + " schedule").c_str(), D.steps, H.steps.data(), sizeof(StepDesc) * H.steps.size());
+        };
+        side("K", lp->K, P.K);
+        side("K'", lp->KT, P.KT);
+        if (lp->k_slots != (int64_t)P.K.col.size() || lp->kt_slots != (int64_t)P.KT.col.size() || lp->k_narrow != P.K.narrow_slots ||
+            lp->kt_narrow != P.KT.narrow_slots || lp->k_long_nnz != (int64_t)P.K.lcol.size() || lp->kt_long_nnz != (int64_t)P.KT.lcol.size())
+            if (why.empty()) why = "slot / narrow / long-row counters";
+        if (!why.empty()) return fail(UC_ERR_INVALID, why);
+    } catch (const CudaFail& f) {
+        return fail(UC_ERR_CUDA, std::string(f.what) + ": " + cudaGetErrorString(f.e));
+    } catch (const std::exception& e) {
+        return fail(UC_ERR_NOMEM, e.what());
+    }
+    return UC_OK;
+}
+
 int uc_lp_get_scaling(uc_lp* lp, double* Dr_out, double* Dc_out) {
     if (!lp) return fail(UC_ERR_INVALID, "handle is NULL");
     try {
@@ -995,12 +1341,16 @@ int uc_lp_get_scaling(uc_lp* lp, double* Dr_out, double* Dc_out) {
         if (Dr_out) {
             t.resize((size_t)lp->m);
             if (lp->m) CK(cudaMemcpy(t.data(), lp->Dr, sizeof(double) * (size_t)lp->m, cudaMemcpyDeviceToHost));
-            for (int64_t k = 0; k < lp->m; ++k) Dr_out[lp->h_perm_r[(size_t)k]] = t[(size_t)k];
+            std::vector<long long> pr((size_t)lp->m);
+            if (lp->m) CK(cudaMemcpy(pr.data(), lp->perm_r, sizeof(long long) * (size_t)lp->m, cudaMemcpyDeviceToHost));
+            for (int64_t k = 0; k < lp->m; ++k) Dr_out[pr[(size_t)k]] = t[(size_t)k];
         }
         if (Dc_out) {
             t.resize((size_t)lp->n);
             if (lp->n) CK(cudaMemcpy(t.data(), lp->Dc, sizeof(double) * (size_t)lp->n, cudaMemcpyDeviceToHost));
-            for (int64_t k = 0; k < lp->n; ++k) Dc_out[lp->h_perm_c[(size_t)k]] = t[(size_t)k];
+            std::vector<long long> pc((size_t)lp->n);
+            if (lp->n) CK(cudaMemcpy(pc.data(), lp->perm_c, sizeof(long long) * (size_t)lp->n, cudaMemcpyDeviceToHost));
+            for (int64_t k = 0; k < lp->n; ++k) Dc_out[pc[(size_t)k]] = t[(size_t)k];
         }
     } catch (const CudaFail& f) {
         return fail(UC_ERR_CUDA, std::string(f.what) + ": " + cudaGetErrorString(f.e));

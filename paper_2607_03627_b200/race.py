@@ -162,9 +162,9 @@ def race(handle: "_b.UcLp", competitor: Callable[..., Any], competitor_args: tup
     return res
 
 
-def highs_competitor(lp):
+def highs_competitor(lp, time_limit=None):
     """Stand-in for the paper's CPU barrier solver: HiGHS through scipy (optional dependency).  Returns the optimal
-    objective of min c'x s.t. Ax {=,>=} b, l <= x <= u."""
+    objective of min c'x s.t. Ax {=,>=} b, l <= x <= u; raises if HiGHS stops for any other reason (`time_limit` s)."""
     import numpy as np
     import scipy.sparse as sp
     from scipy.optimize import linprog
@@ -177,31 +177,71 @@ def highs_competitor(lp):
         kw.update(A_ub=-A[G], b_ub=-lp.b[G])
     if E.any():
         kw.update(A_eq=A[E], b_eq=lp.b[E])
-    r = linprog(lp.c, bounds=bounds, method="highs", **kw)
+    r = linprog(lp.c, bounds=bounds, method="highs", options=({"time_limit": float(time_limit)} if time_limit else None), **kw)
     if r.status != 0:
         raise RuntimeError(r.message)
     return float(r.fun)
 
 
+def cancel_latency(handle, after_s: float = 0.2, repeats: int = 5, **solve_kwargs):
+    """Seconds between uc_pdhg_cancel and the return of a uc_pdhg_solve that is in full flight (`after_s` after its
+    start, with tolerances it cannot reach): what Algorithm 1's "terminate the other solver" (P:l.82-84) costs on the
+    GPU side.  Returns the list of measured latencies and the attempts each cancelled solve had run."""
+    lat, its = [], []
+    for _ in range(repeats):
+        box = {}
+        th = threading.Thread(target=lambda: box.update(sol=handle.solve(eps_rel=0.0, eps_abs=0.0, iter_limit=10**9, **solve_kwargs)), daemon=True)
+        th.start()
+        time.sleep(after_s)
+        t = time.perf_counter()
+        handle.cancel()
+        th.join()
+        lat.append(time.perf_counter() - t)
+        assert box["sol"].status == _b.CANCELLED, _b.STATUS_NAMES.get(box["sol"].status)
+        its.append(box["sol"].iterations)
+    return lat, its
+
+
 def _main():
-    """python -m paper_2607_03627_b200.race --configs 0 1 [--poll 0.05] [--alone-limit-s 600]: one table row per UC config."""
+    """python -m paper_2607_03627_b200.race --configs 0 1 2 [--poll 0.5] [--eps-abs 1e-4 1e-5] [--cancel-config 3]:
+    a Table-VI-style row per UC config and tolerance (which pipeline wins, P:l.221-226), with the CPU cores split evenly
+    between the two pipelines (P:l.70), then the cancel latency of a solve in full flight."""
     import argparse
     from workloads import uc_config
     ap = argparse.ArgumentParser()
     ap.add_argument("--configs", type=int, nargs="+", default=[0, 1])
-    ap.add_argument("--poll", type=float, default=0.05)
+    ap.add_argument("--poll", type=float, default=0.5, help="poll period in s (0.5 in the paper, P:l.81)")
+    ap.add_argument("--eps-abs", type=float, nargs="+", default=[1e-4], help="absolute tolerance(s); 1e-5 is the paper's knob (P:l.66)")
+    ap.add_argument("--cancel-config", type=int, default=None)
+    ap.add_argument("--alone-limit-s", type=float, default=120.0, help="time limit of the stand-alone HiGHS run of the table")
     args = ap.parse_args()
-    print("| config | winner | race s | GPU PDHG alone s (attempts) | HiGHS alone s | objective | cancel latency ms |")
-    print("|---|---|---|---|---|---|---|")
+    gpu_cores, cpu_cores = partition_cores()
+    print(f"cores: GPU pipeline host thread {len(gpu_cores)}, CPU competitor {len(cpu_cores)}; poll {args.poll} s")
+    print("| config | eps_abs | winner | race s | GPU PDHG alone s (attempts) | HiGHS alone s | objective | cancel latency ms |")
+    print("|---|---|---|---|---|---|---|---|")
     for c in args.configs:
         lp = uc_config(c)
+        t = time.perf_counter()
+        try:
+            highs_competitor(lp, args.alone_limit_s); tcs = f"{time.perf_counter() - t:.2f}"
+        except RuntimeError:
+            tcs = f"> {args.alone_limit_s:g} (time limit)"
         with _b.UcLp(lp) as h:
             h.solve(fixed_iterations=64)                  # warm-up: graph instantiation is not part of the race
-            r = race(h, highs_competitor, (lp,), poll_s=args.poll)
-            t = time.perf_counter(); s = h.solve(); tg = time.perf_counter() - t
-        t = time.perf_counter(); highs_competitor(lp); tc = time.perf_counter() - t
-        lat = "-" if r.cancel_latency_s is None else f"{1e3 * r.cancel_latency_s:.1f}"
-        print(f"| {c} | {r.winner} | {r.seconds:.2f} | {tg:.3f} ({s.iterations}) | {tc:.2f} | {r.objective:.4f} | {lat} |", flush=True)
+            for ea in args.eps_abs:
+                kw = dict(eps_abs=ea)
+                r = race(h, highs_competitor, (lp,), poll_s=args.poll, solve_kwargs=kw, cpu_cores=cpu_cores, gpu_host_cores=gpu_cores)
+                t = time.perf_counter(); s = h.solve(**kw); tg = time.perf_counter() - t
+                lat = "-" if r.cancel_latency_s is None else f"{1e3 * r.cancel_latency_s:.1f}"
+                print(f"| {c} | {ea:g} | {r.winner} | {r.seconds:.2f} | {tg:.3f} ({s.iterations}) | {tcs} | {r.objective:.4f} | {lat} |", flush=True)
+    if args.cancel_config is not None:
+        lp = uc_config(args.cancel_config)
+        with _b.UcLp(lp) as h:
+            h.solve(fixed_iterations=64)
+            lat, its = cancel_latency(h)
+        print()
+        print(f"cancel latency on config {args.cancel_config} (solve in full flight, cancelled 0.2 s after its start): "
+              + ", ".join(f"{1e3 * v:.1f}" for v in lat) + f" ms; attempts run: {its}")
 
 
 if __name__ == "__main__":

@@ -87,6 +87,57 @@ def assert_trajectory_parity(lp, F=200, **opts):
     return sg, so
 
 
+# ------------------------------------------------------------------ A1: ingest on the device (integer work: bit-exact)
+def banded_and_wide_lp(n=60_000, m=45_000, seed=4):
+    """Narrow-band rows (16-bit offsets apply) mixed with rows that reach across all columns (32-bit slices)."""
+    from workloads.lp import from_coo
+    rng = np.random.default_rng(seed)
+    rows, cols = [], []
+    for i in range(m):
+        k = int(rng.integers(1, 6))
+        if i % 97 == 0:
+            c = rng.choice(n, size=k, replace=False)
+        else:
+            base = int(i * (n - 300) / m)
+            c = base + rng.choice(300, size=k, replace=False)
+        rows += [i] * k; cols += c.tolist()
+    vals = rng.standard_normal(len(rows))
+    return from_coo(m, n, rows, cols, vals, np.full(m, ord("G"), np.uint8), -np.ones(m), rng.standard_normal(n), -np.ones(n), np.ones(n), name="banded")
+
+
+INGEST_CASES = dict(CASES, banded=banded_and_wide_lp, random_3e5=lambda: random_lp(300_000, 22), uc2=lambda: uc_config(2))
+
+
+@pytest.mark.parametrize("name", list(INGEST_CASES))
+@pytest.mark.parametrize("window,thr,compress", [(4096, 32, 1), (64, 3, 1), (4096, 1000, 0)])
+def test_device_ingest_builds_the_host_layouts_bit_for_bit(name, window, thr, compress):
+    """uc_lp_create with host_ingest = 0 (kernels: stable radix sorts, scans, per-row fills) must leave on the device
+    exactly what the host builders -- verified against the caller's CSR by uc_host_layout_selftest -- produce:
+    permutations, slice pointers, 32-bit indices / 16-bit offsets, values, long rows, schedules.  No preconditioning,
+    so that the values can be compared too."""
+    if name not in INGEST_CASES:
+        pytest.skip()
+    lp = INGEST_CASES[name]() if name not in CASES else get_lp(name)
+    with P.UcLp(lp, sell_window=window, long_row_threshold=thr, index_compression=compress, ruiz_iters=0, pc_alpha=0.0, host_ingest=0) as h:
+        h.compare_layout(lp)
+    with P.UcLp(lp, sell_window=window, long_row_threshold=thr, index_compression=compress, ruiz_iters=0, pc_alpha=0.0, host_ingest=1) as h:
+        h.compare_layout(lp)                                  # the checker agrees with itself through the upload path
+
+
+def test_device_and_host_ingest_give_identical_solves():
+    lp = get_lp("uc1")
+    with P.UcLp(lp, host_ingest=0) as a, P.UcLp(lp, host_ingest=1) as b:
+        sa = a.solve(fixed_iterations=200, trace_attempts=200); sb = b.solve(fixed_iterations=200, trace_attempts=200)
+    np.testing.assert_array_equal(sa.x, sb.x); np.testing.assert_array_equal(sa.y, sb.y)
+    np.testing.assert_array_equal(sa.attempts["eta_used"], sb.attempts["eta_used"])
+
+
+def test_paper_scale_config3_device_ingest_matches_host_layouts():
+    lp = uc_config(3)
+    with P.UcLp(lp, ruiz_iters=0, pc_alpha=0.0) as h:
+        h.compare_layout(lp)
+
+
 # ------------------------------------------------------------------ R1: preconditioner + layouts
 @pytest.mark.parametrize("name", ["two_var", "small_random", "ragged", "uc0", "uc1", "random_2e4"])
 def test_preconditioner_matches_oracle(name):
@@ -112,6 +163,29 @@ def test_preconditioner_options(alpha, ruiz):
     np.testing.assert_allclose(gDc, Dc, rtol=1e-14)
 
 
+@pytest.mark.parametrize("alpha,ruiz", [(0.5, 10), (1.5, 2)])
+def test_pock_chambolle_general_exponent(alpha, ruiz):
+    """alpha != 1 takes the `pow` branch of k_row_stat (mode 2).  CUDA's pow is 2-ulp accurate where the oracle's libm pow
+    is correctly rounded, so the bar is not bit equality: a sum of positive terms keeps the relative error of its terms
+    (<= 2 ulp = 4.4e-16), the square root halves it and the division by r_i * s_j adds both: < 1e-15 per value; 1e-13
+    leaves room for the ordering of the sums.  The two layouts must still agree bit for bit (same r_i * s_j in both).
+    The trajectories are then NOT bit-identical (the scaled problems differ in the last bits), so the two solves stop at
+    different points of the same 1e-4 relative KKT ball: their objectives agree to that accuracy, not to 1e-5."""
+    lp = get_lp("uc0")
+    vs, Dr, Dc = oracle.precondition(lp, ruiz_iters=ruiz, pc_alpha=alpha)
+    with P.UcLp(lp, keep_source_map=1, ruiz_iters=ruiz, pc_alpha=alpha) as h:
+        gDr, gDc = h.scaling()
+        v_k, v_kt = h.scaled_values(False), h.scaled_values(True)
+        sg = h.solve()
+    np.testing.assert_allclose(v_k, vs, rtol=1e-13)
+    np.testing.assert_allclose(gDr, Dr, rtol=1e-13)
+    np.testing.assert_allclose(gDc, Dc, rtol=1e-13)
+    np.testing.assert_array_equal(v_k, v_kt)
+    so = oracle.solve(lp, ruiz_iters=ruiz, pc_alpha=alpha)
+    assert sg.status == P.OPTIMAL and so.status == 0 and sg.rel_kkt <= 1e-4
+    assert abs(sg.primal_obj - so.primal_obj) <= 5e-4 * abs(so.primal_obj)
+
+
 @pytest.mark.parametrize("name", ["small_random", "ragged", "uc1"])
 def test_spmv_pair_matches_oracle_and_is_adjoint(name):
     lp = get_lp(name)
@@ -124,6 +198,44 @@ def test_spmv_pair_matches_oracle_and_is_adjoint(name):
     ox, oty = oracle.spmv(lp, x, val=vs), oracle.spmv_t(lp, y, val=vs)
     assert rel_l2(kx, ox) <= 1e-13 and rel_l2(kty, oty) <= 1e-13
     assert abs(y @ kx - kty @ x) <= 1e-12 * (np.abs(y) @ np.abs(kx) + 1.0)       # adjoint identity
+
+
+# ------------------------------------------------------------------ A5..A9 at kernel level: ONE attempt, restated in numpy
+@pytest.mark.parametrize("name", ["small_random", "ragged", "uc0", "uc1", "random_2e4"])
+def test_one_attempt_of_the_attempt_kernels_matches_a_numpy_restatement(name):
+    """k_primal + k_dual once, from a random warm start, against R2..R5 written out with scipy on the oracle's scaled
+    matrix: g = K~'y~, x' = clamp(x~ - tau (c~ - g)), xbar = 2x' - x~, y' = proj(y~ + sigma (q~ - K~ xbar)) and the three
+    reductions of the step rule.  This is the kernel-level tier for the pipelines of uc_attempt.cuh (uc_lp_spmv runs the
+    check kernels' traversal, not these)."""
+    import scipy.sparse as sp
+    lp = get_lp(name)
+    rng = np.random.default_rng(11)
+    x0 = rng.standard_normal(lp.n); y0 = rng.standard_normal(lp.m)
+    vs, Dr, Dc = oracle.precondition(lp)
+    K = sp.csr_matrix((vs, lp.col_idx, lp.row_ptr), shape=(lp.m, lp.n))
+    isG = np.asarray(lp.sense) == ord("G")
+    c, q = lp.c / Dc, lp.b / Dr
+    l = np.where(lp.l <= -1e20, -np.inf, lp.l * Dc); u = np.where(lp.u >= 1e20, np.inf, lp.u * Dc)
+    x = np.clip(x0 * Dc, l, u); y = y0 * Dr; y[isG] = np.maximum(y[isG], 0.0)                      # R2
+    eta = 1.0 / np.abs(vs).max() if lp.nnz else 1.0
+    nc, nq = np.linalg.norm(c), np.linalg.norm(q)
+    omega = nc / nq if nc > 1e-10 and nq > 1e-10 else 1.0
+    xn = np.clip(x - (eta / omega) * (c - K.T @ y), l, u); xbar = 2.0 * xn - x                       # R3
+    yn = y + eta * omega * (q - K @ xbar); yn[isG] = np.maximum(yn[isG], 0.0)                       # R4
+    dx, dy = xn - x, yn - y
+    dx2, dy2, inter = float(dx @ dx), float(dy @ dy), abs(float(dy @ (K @ dx)))                     # R5
+    with P.UcLp(lp) as h:
+        s = h.solve(x0=x0, y0=y0, fixed_iterations=1, trace_attempts=1)
+    a = s.attempts[0]
+    assert a["eta_used"] == pytest.approx(eta, rel=1e-14)
+    assert a["dx2"] == pytest.approx(dx2, rel=1e-12) and a["dy2"] == pytest.approx(dy2, rel=1e-12)
+    assert a["inter"] == pytest.approx(inter, rel=1e-9, abs=1e-12 * (dx2 + dy2))
+    N = omega * dx2 + dy2 / omega
+    assert bool(a["accepted"]) == (eta <= (N / (2 * inter) if inter > 0 else np.inf))
+    ex, ey = (xn, yn) if a["accepted"] else (x, y)
+    assert rel_l2(s.x, ex / Dc) <= 1e-12
+    if lp.m:
+        assert rel_l2(s.y, ey / Dr) <= 1e-12
 
 
 # ------------------------------------------------------------------ R2..R11: 200-attempt trajectory
