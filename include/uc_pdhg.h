@@ -81,6 +81,8 @@ void uc_lp_default_options(uc_lp_options* opt);
  *   b[m], c[n]       finite;  l[n], u[n]: l <= u, -INFINITY / +INFINITY or |v| >= 1e20 = absent (R13)
  *   opt              NULL = defaults
  *   out              receives the handle
+ * The call keeps its block of scratch device memory (the caller's CSR and the sort buffers of the ingest kernels, ~150
+ * bytes per nonzero, at most 2 GiB) cached per device in the process for the next uc_lp_create; larger blocks are freed.
  */
 int uc_lp_create(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, const int32_t* col_idx,
                  const double* val, const char* sense, const double* b, const double* c, const double* l,

@@ -6,7 +6,9 @@ import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-LIB = os.path.join(HERE, "libuc_pdhg.so")
+# UC_PDHG_LIB: load another build of the same sources instead (e.g. the -DUC_DEBUG_BOUNDS build for a checking run of
+# the GPU tests); it is never built or rebuilt from here
+LIB = os.environ.get("UC_PDHG_LIB") or os.path.join(HERE, "libuc_pdhg.so")
 SOURCES = [os.path.join(CSRC, "uc_pdhg.cu")]
 DEPENDS = SOURCES + [os.path.join(CSRC, "uc_kernels.cuh"), os.path.join(CSRC, "uc_attempt.cuh"), os.path.join(CSRC, "uc_dd.cuh"), os.path.join(CSRC, "uc_format.hpp"),
                      os.path.join(os.path.dirname(HERE), "include", "uc_pdhg.h")]
@@ -22,6 +24,8 @@ def nvcc() -> str:
 
 
 def stale() -> bool:
+    if os.environ.get("UC_PDHG_LIB"):
+        return False
     if not os.path.exists(LIB):
         return True
     t = os.path.getmtime(LIB)
@@ -30,7 +34,7 @@ def stale() -> bool:
 
 def build(force: bool = False, verbose: bool = False) -> str:
     """Compile the CUDA extension if it is missing or older than its sources; returns the .so path."""
-    if force or stale():
+    if (force and not os.environ.get("UC_PDHG_LIB")) or stale():
         tmp = LIB + f".tmp{os.getpid()}"
         cmd = [nvcc(), *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), "-o", tmp, *SOURCES]
         subprocess.check_call(cmd)

@@ -352,7 +352,6 @@ __global__ void __launch_bounds__(kPrimalThreads, kCtasPerSm) k_primal(Sell KT, 
     extern __shared__ __align__(128) unsigned char smem_raw[];
     PrimalSmem& P = *reinterpret_cast<PrimalSmem*>(smem_raw);
     dd* const red = P.red;
-    grid_launch_dependents();
     UC_TL_MARK(V, 0);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     dd acc[1] = {dd{0.0, 0.0}};
@@ -364,6 +363,9 @@ __global__ void __launch_bounds__(kPrimalThreads, kCtasPerSm) k_primal(Sell KT, 
                                                        // vector v = 2k + lane/16, doubles off, off+1; vkey 0: copy it
     auto dep_ready = [&]() -> bool {
         grid_dependency_wait();
+        // only now may the next k_dual start: the k_dual before this kernel has completed, so the control block it left
+        // is final and the next k_dual may read it BEFORE its own dependency (this kernel) resolves
+        grid_launch_dependents();
         UC_TL_MARK(V, 1);
         const CtrlHot h = load_hot(ctl);
         if (h.done) return false;
@@ -437,7 +439,6 @@ __global__ void __launch_bounds__(kDualThreads, kCtasPerSm) k_dual(Sell K, Vecs 
     dd acc[2] = {dd{0.0, 0.0}, dd{0.0, 0.0}};
     const Policies pol{policy_evict_first(), policy_evict_last()};
     const double2* xg = V.xg;
-    // everything below is set by dep_ready(), i.e. read after the previous kernel has completed
     int cur = 0, pend = 0; double eta_prev = 0.0, sig = 0.0;
     const double* ycur = nullptr; double* ynext = nullptr;
     const double* vsrc[2]; int voff[2]; int vkey[2];   // this lane's share of a slice's vector segments (vkey 0: copy it)
@@ -447,26 +448,29 @@ __global__ void __launch_bounds__(kDualThreads, kCtasPerSm) k_dual(Sell K, Vecs 
     // whole solve
     struct RuleIn { double eta, omega, w; long long k, acc, cap; double2 pw; uc_attempt_record* att; };
     __shared__ RuleIn rule_in;
+    // The control block is read HERE, before the dependency on k_primal resolves: k_primal does not write it, and the
+    // k_dual that did has completed (k_primal lets this kernel start only after its own dependency resolved).  One L2
+    // round trip less on the serial path of every attempt.
+    const CtrlHot h = load_hot(ctl);
+    cur = h.cur; pend = h.pending; eta_prev = h.eta_prev; sig = h.eta * h.omega;
+    if (threadIdx.x == K.cta_warps * 32 && !h.done) {      // the long-row warp: its dependent loads delay no slice
+        RuleIn r;
+        r.eta = h.eta; r.omega = h.omega; r.w = h.w; r.k = ctl->k; r.acc = ctl->accepted;
+        r.att = ctl->att; r.cap = ctl->att_cap; r.pw = ctl->powtab[r.k];     // {(k+1)^-0.6, (k+1)^-0.3} of attempt k = r.k + 1
+        rule_in = r;
+    }
+    ycur = V.y[cur]; ynext = V.y[cur ^ 1];
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+        const int v = 2 * k + (lane >> 4), off = (lane & 15) * 2;
+        vsrc[k] = (v == 0 ? ycur : v == 1 ? V.q : V.ysum) + off;
+        voff[k] = v * 32 + off; vkey[k] = (v < 2 || (v == 2 && pend)) ? 0 : 1;
+    }
+    const bool solve_over = h.done != 0;
     auto dep_ready = [&]() -> bool {
         grid_dependency_wait();
         UC_TL_MARK(V, 1);
-        const CtrlHot h = load_hot(ctl);
-        if (h.done) return false;
-        cur = h.cur; pend = h.pending; eta_prev = h.eta_prev; sig = h.eta * h.omega;
-        if (threadIdx.x == K.cta_warps * 32) {             // the long-row warp: its dependent loads delay no slice
-            RuleIn r;
-            r.eta = h.eta; r.omega = h.omega; r.w = h.w; r.k = ctl->k; r.acc = ctl->accepted;
-            r.att = ctl->att; r.cap = ctl->att_cap; r.pw = ctl->powtab[r.k];     // {(k+1)^-0.6, (k+1)^-0.3} of attempt k = r.k + 1
-            rule_in = r;
-        }
-        ycur = V.y[cur]; ynext = V.y[cur ^ 1];
-#pragma unroll
-        for (int k = 0; k < 2; ++k) {
-            const int v = 2 * k + (lane >> 4), off = (lane & 15) * 2;
-            vsrc[k] = (v == 0 ? ycur : v == 1 ? V.q : V.ysum) + off;
-            voff[k] = v * 32 + off; vkey[k] = (v < 2 || (v == 2 && pend)) ? 0 : 1;
-        }
-        return true;
+        return !solve_over;
     };
 
     if (warp == K.cta_warps) {                              // ---- long rows

@@ -82,8 +82,9 @@ struct HostSell {
 //   2. Inside its range a CTA deals the slices, in ascending order, to its warp with the least estimated work so far
 //      (ties: lowest warp), so that its warps finish together while, at any moment, they work on neighbouring slices
 //      (one shared working set in L1).
-// The estimate is in units of ~100 cycles from the measured per-step breakdown: 7 per step +
-// 1.3 per entry per row + 4 for the step that applies the update.  A warp takes its slices in ascending order, each as
+// The estimate (7 per step + 1.3 per entry per row + 4 for the step that applies the update, in units of ~100 cycles) was
+// fitted in round 1 to per-warp cycle counters of a scratch build that is not in this tree; what IS reproducible is its
+// result: the spread of the warps' busy times that python -m paper_2607_03627_b200.timeline prints (profiles/).  A warp takes its slices in ascending order, each as
 // ceil(width / kChunkT) steps.  Stored step-major, steps[j * warps + w] with w = cta * warps_per_cta + warp, padded with
 // empty steps to the longest warp, so that step j of all warps is one coalesced read.  The assignment is fixed at
 // create time: solves are reproducible bit for bit.

@@ -717,11 +717,12 @@ __global__ void __launch_bounds__(kBlock) k_reduce(const double* v, long long n,
         if (threadIdx.x == 0) part[blockIdx.x] = a[0];
     }
 }
-__global__ void k_reduce_final(const dd* part, int count, int op, double* out) {
-    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+__global__ void k_reduce_final(const dd* part, int count, int op, double* out) {     // one warp
+    if (blockIdx.x != 0 || threadIdx.x >= 32) return;
     dd a = dd{0.0, 0.0};
-    for (int i = 0; i < count; ++i) { if (op) a.hi = fmax(a.hi, part[i].hi); else a = dd_add(a, part[i]); }
-    *out = dd_round(a);
+    for (int i = threadIdx.x; i < count; i += 32) { if (op) a.hi = fmax(a.hi, part[i].hi); else a = dd_add(a, part[i]); }
+    if (op) a.hi = warp_max(a.hi); else a = warp_sum_dd(a);
+    if (threadIdx.x == 0) *out = dd_round(a);
 }
 
 // plain SpMV with the solver's traversal (test hook uc_lp_spmv)

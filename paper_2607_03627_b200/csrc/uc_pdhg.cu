@@ -54,6 +54,10 @@ struct uc_lp {
     Vecs V{};
     Ctrl* ctl = nullptr;
     double *Dr = nullptr, *Dc = nullptr;   // writable aliases of V.Dr / V.Dc
+    // device staging of the host-buffer entry point (uc_pdhg_solve): results before they go to the caller's buffers, and a
+    // warm start after it came from them.  Owned by the handle: no cudaMalloc / cudaFree on the solve path (they
+    // synchronise the device and were seen to stall for hundreds of ms now and then).
+    double *stage_x = nullptr, *stage_y = nullptr, *stage_x0 = nullptr, *stage_y0 = nullptr;
     double *qs = nullptr, *cs = nullptr, *ls = nullptr, *us = nullptr;
     unsigned char* isG = nullptr;
     // host <-> device mailboxes (pinned, mapped)
@@ -166,9 +170,37 @@ Sell upload_sell(uc_lp* lp, const HostSell& H) {
 // ------------------------------------------------------------------------------------------ A1 on the device
 // Temporary device memory of uc_lp_create: one allocation, bump-allocated, released when create returns.
 struct TempArena {
-    char* base = nullptr; size_t cap = 0, used = 0;
-    ~TempArena() { if (base) cudaFree(base); }
-    void reserve(size_t bytes) { CK(cudaMalloc((void**)&base, bytes)); cap = bytes; }
+    // One block, bump-allocated.  The block is kept in a per-device cache of this process when uc_lp_create returns (up to
+    // kScratchKeep bytes; a larger one is freed) and reused by the next uc_lp_create: cudaMalloc / cudaFree of ~1 GB
+    // synchronise the device and were seen to stall for 0.1-0.6 s now and then -- more than the whole of uc_lp_create.
+    // (A stream-ordered pool was measured too: its first ~1 GB allocation costs 0.35 s.)
+    static constexpr size_t kScratchKeep = (size_t)2 << 30;
+    struct Cache { std::mutex mu; std::vector<void*> base; std::vector<size_t> cap; std::vector<char> busy; };
+    static Cache& cache() { static Cache c; return c; }
+    char* base = nullptr; size_t cap = 0, used = 0; int dev = -1; bool cached = false;
+    ~TempArena() {
+        if (!base) return;
+        Cache& C = cache();
+        std::lock_guard<std::mutex> g(C.mu);
+        if (cached) { C.busy[(size_t)dev] = 0; return; }                     // back to the cache
+        if (cap <= kScratchKeep && !C.busy[(size_t)dev]) {                   // becomes the cache (the smaller old one goes)
+            if (C.base[(size_t)dev]) cudaFree(C.base[(size_t)dev]);
+            C.base[(size_t)dev] = base; C.cap[(size_t)dev] = cap;
+        } else cudaFree(base);
+    }
+    void reserve(size_t bytes, int device) {
+        dev = device;
+        Cache& C = cache();
+        {
+            std::lock_guard<std::mutex> g(C.mu);
+            if ((int)C.base.size() <= dev) { C.base.resize((size_t)dev + 1, nullptr); C.cap.resize((size_t)dev + 1, 0); C.busy.resize((size_t)dev + 1, 0); }
+            if (!C.busy[(size_t)dev] && C.base[(size_t)dev] && C.cap[(size_t)dev] >= bytes) {
+                base = (char*)C.base[(size_t)dev]; cap = C.cap[(size_t)dev]; C.busy[(size_t)dev] = 1; cached = true;
+                return;
+            }
+        }
+        CK(cudaMalloc((void**)&base, bytes)); cap = bytes;
+    }
     template <class T> T* get(size_t count) {
         const size_t bytes = ((count * sizeof(T) + 255) / 256 + 1) * 256;
         if (used + bytes > cap) throw CudaFail{cudaErrorMemoryAllocation, "temporary arena of uc_lp_create"};
@@ -461,8 +493,7 @@ void destroy_impl(uc_lp* lp) {
     if (lp->ev_t1) cudaEventDestroy(lp->ev_t1);
     for (void* p : lp->allocs) if (p) cudaFree(p);
     if (lp->powtab) cudaFree(lp->powtab);
-    if (lp->h_status) cudaFreeHost(lp->h_status);
-    if (lp->h_stop) cudaFreeHost(lp->h_stop);
+    if (lp->h_status) cudaFreeHost(lp->h_status);        // one allocation: the stop flag lives behind the status record
     if (lp->own_stream) cudaStreamDestroy(lp->own_stream);
     delete lp;
 }
@@ -491,6 +522,7 @@ int uc_host_layout_selftest(int64_t m, int64_t n, int64_t nnz, const int64_t* ro
                             int32_t sell_window, int32_t long_row_threshold, int32_t sched_ctas, int32_t warps_per_cta) {
     if (m < 0 || n < 0 || nnz < 0 || !row_ptr || sell_window < 32 || long_row_threshold < 1 || sched_ctas < 1 || warps_per_cta < 1)
         return fail(UC_ERR_INVALID, "bad argument");
+    try {
     HostProblem P;
     build_perms(m, n, nnz, row_ptr, col_idx, sell_window, long_row_threshold, P);
     build_K(row_ptr, col_idx, val, true, P);
@@ -640,6 +672,9 @@ int uc_host_layout_selftest(int64_t m, int64_t n, int64_t nnz, const int64_t* ro
     if (!w.empty()) return bad("K layout: " + w);
     w = check_sell(P.KT, true);
     if (!w.empty()) return bad("K' layout: " + w);
+    } catch (const std::exception& e) {                        // nothing may unwind through the C ABI
+        return fail(UC_ERR_NOMEM, std::string("uc_host_layout_selftest: ") + e.what());
+    }
     return UC_OK;
 }
 
@@ -721,10 +756,17 @@ int uc_lp_create(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, cons
             attempt_shape(nshort_r, m - nshort_r, kDualWarps, gridPB, warpsPB);
         };
         int gridPA = 1, gridPB = 1;
-        TempArena T;                                               // released when create returns
-        // the data vectors (original order, temporary) go up on a helper thread with its own stream, next to the CSR
-        TempArena TV;
-        TV.reserve((size_t)8 * (size_t)(m + 3 * n) + (size_t)m + 8 * 512 + sizeof(dd) * 1024 + 4096);
+        // temporaries of this call: the data vectors in the caller's order, and (device ingest) the caller's CSR with
+        // everything the ingest kernels and sorts need
+        TempArena T;
+        {
+            const size_t vec_bytes = (size_t)8 * (size_t)(m + 3 * n) + (size_t)m + 8 * 512 + sizeof(dd) * 1024 + 4096;
+            const size_t src_bytes = want_src ? 16 * ((size_t)nnz + 32 * (size_t)(m + n) / 32 + 1024) * 3 : 0;
+            const size_t ingest_bytes = opt.host_ingest ? 0 : (size_t)(8 * (m + 1) + 44 * nnz + 28 * n + 4 * m + 44 * (m + n)) +
+                                        ((size_t)(m + n) / 32 + 2) * 40 + src_bytes + 256 * 64 + ((size_t)64 << 20);
+            T.reserve(vec_bytes + ingest_bytes, dev);
+        }
+        TempArena& TV = T;
         double* db = TV.get<double>((size_t)m + 1); double* dc = TV.get<double>((size_t)n + 1);
         double* dl = TV.get<double>((size_t)n + 1); double* du = TV.get<double>((size_t)n + 1);
         char* dsense = TV.get<char>((size_t)m + 1);
@@ -744,9 +786,6 @@ int uc_lp_create(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, cons
         phase("stream/events");
         if (!opt.host_ingest) {
             // ---- A1 on the device (uc_ingest.cuh): one copy of the caller's CSR, then kernels
-            const size_t src_bytes = want_src ? 16 * ((size_t)nnz + 32 * (size_t)(m + n) / 32 + 1024) * 3 : 0;
-            T.reserve((size_t)(8 * (m + 1) + 44 * nnz + 28 * n + 4 * m + 44 * (m + n)) + ((size_t)(m + n) / 32 + 2) * 40 +
-                      src_bytes + 256 * 64 + ((size_t)64 << 20));
             long long* d_ptr = T.get<long long>((size_t)m + 1);
             int* d_col = T.get<int>((size_t)nnz + 1);
             double* d_val = T.get<double>((size_t)nnz + 1);
@@ -846,11 +885,12 @@ int uc_lp_create(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, cons
         lp->K.ncols = n; lp->KT.ncols = m; lp->K.cta_warps = warpsPB; lp->KT.cta_warps = warpsPA;
         Vecs& V = lp->V;
         V.n = n; V.m = m;
-        lp->reserve_arena((size_t)(11 * 8 + 16) * (size_t)(n + 64) + (size_t)(7 * 8 + 1) * (size_t)(m + 64) + ((size_t)1 << 20));
+        lp->reserve_arena((size_t)(13 * 8 + 16) * (size_t)(n + 64) + (size_t)(9 * 8 + 1) * (size_t)(m + 64) + ((size_t)1 << 20));   // incl. the four staging vectors
         for (int i = 0; i < 2; ++i) { V.x[i] = lp->dalloc<double>((size_t)n); V.y[i] = lp->dalloc<double>((size_t)m); }
         V.xg = lp->dalloc<double2>((size_t)n);
         V.xsum = lp->dalloc<double>((size_t)n); V.ysum = lp->dalloc<double>((size_t)m);
         V.xr = lp->dalloc<double>((size_t)n); V.yr = lp->dalloc<double>((size_t)m);
+        lp->stage_x = lp->dalloc<double>((size_t)n); lp->stage_y = lp->dalloc<double>((size_t)m);
         lp->cs = lp->dalloc<double>((size_t)n); lp->ls = lp->dalloc<double>((size_t)n); lp->us = lp->dalloc<double>((size_t)n);
         lp->qs = lp->dalloc<double>((size_t)m); lp->isG = lp->dalloc<unsigned char>((size_t)m);
         lp->Dr = lp->dalloc<double>((size_t)m); lp->Dc = lp->dalloc<double>((size_t)n);
@@ -872,9 +912,12 @@ int uc_lp_create(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, cons
         V.partR = lp->dalloc<dd>((size_t)2 * V.gridR);
         lp->ctl = lp->dalloc<Ctrl>(1);
         CK(cudaMemsetAsync(lp->ctl, 0, sizeof(Ctrl), st));
-        CK(cudaHostAlloc((void**)&lp->h_status, sizeof(HostStatus), cudaHostAllocMapped));
-        CK(cudaHostAlloc((void**)&lp->h_stop, sizeof(int), cudaHostAllocMapped));
-        std::memset(lp->h_status, 0, sizeof(HostStatus)); *lp->h_stop = 0;
+        // the two host <-> device mailboxes share ONE mapped pinned allocation (the status record, then the stop flag on
+        // its own 128-byte line): pinned allocations and their release are slow, synchronising driver calls
+        static_assert(sizeof(HostStatus) <= 128, "mailbox layout");
+        CK(cudaHostAlloc((void**)&lp->h_status, 256, cudaHostAllocMapped));
+        lp->h_stop = reinterpret_cast<int*>(reinterpret_cast<char*>(lp->h_status) + 128);
+        std::memset(lp->h_status, 0, 256);
         CK(cudaHostGetDevicePointer((void**)&lp->d_status, lp->h_status, 0));
         CK(cudaHostGetDevicePointer((void**)&lp->d_stop, lp->h_stop, 0));
 
@@ -1004,7 +1047,6 @@ static int solve_impl(uc_lp* lp, const uc_pdhg_params* pin, double* x_out, doubl
     const double t_wall = now_s();
     int rc = UC_OK;
     bool in_flight = false;
-    double *tx0 = nullptr, *ty0 = nullptr, *tx = nullptr, *ty = nullptr;
     uc_attempt_record* d_att = nullptr; uc_check_record* d_chk = nullptr;
     try {
         DeviceGuard guard(lp->device);
@@ -1033,11 +1075,17 @@ static int solve_impl(uc_lp* lp, const uc_pdhg_params* pin, double* x_out, doubl
         const double *dx0 = nullptr, *dy0 = nullptr;
         if (prm.x0) {
             if (dev_io) dx0 = prm.x0;
-            else { CK(cudaMalloc((void**)&tx0, sizeof(double) * (size_t)std::max<long long>(n, 1))); CK(cudaMemcpyAsync(tx0, prm.x0, sizeof(double) * (size_t)n, cudaMemcpyHostToDevice, st)); dx0 = tx0; }
+            else {
+                if (!lp->stage_x0) lp->stage_x0 = lp->dalloc<double>((size_t)n);      // first warm start on this handle; kept
+                CK(cudaMemcpyAsync(lp->stage_x0, prm.x0, sizeof(double) * (size_t)n, cudaMemcpyHostToDevice, st)); dx0 = lp->stage_x0;
+            }
         }
         if (prm.y0) {
             if (dev_io) dy0 = prm.y0;
-            else { CK(cudaMalloc((void**)&ty0, sizeof(double) * (size_t)std::max<long long>(m, 1))); CK(cudaMemcpyAsync(ty0, prm.y0, sizeof(double) * (size_t)m, cudaMemcpyHostToDevice, st)); dy0 = ty0; }
+            else {
+                if (!lp->stage_y0) lp->stage_y0 = lp->dalloc<double>((size_t)m);
+                CK(cudaMemcpyAsync(lp->stage_y0, prm.y0, sizeof(double) * (size_t)m, cudaMemcpyHostToDevice, st)); dy0 = lp->stage_y0;
+            }
         }
         if (prm.attempt_trace && prm.attempt_trace_cap > 0) CK(cudaMalloc((void**)&d_att, sizeof(uc_attempt_record) * (size_t)prm.attempt_trace_cap));
         if (prm.check_trace && prm.check_trace_cap > 0) CK(cudaMalloc((void**)&d_chk, sizeof(uc_check_record) * (size_t)prm.check_trace_cap));
@@ -1089,14 +1137,14 @@ static int solve_impl(uc_lp* lp, const uc_pdhg_params* pin, double* x_out, doubl
         // ---- A14: unscale, un-permute, hand back
         double* ox = x_out; double* oy = y_out;
         if (!dev_io) {
-            if (x_out) { CK(cudaMalloc((void**)&tx, sizeof(double) * (size_t)std::max<long long>(n, 1))); ox = tx; }
-            if (y_out) { CK(cudaMalloc((void**)&ty, sizeof(double) * (size_t)std::max<long long>(m, 1))); oy = ty; }
+            if (x_out) ox = lp->stage_x;
+            if (y_out) oy = lp->stage_y;
         }
         if (ox || oy) { k_output<<<lp->V.gridR, kBlock, 0, st>>>(lp->V, lp->ctl, ox, oy, lp->perm_c, lp->perm_r); launches += 1; }
         CK(cudaGetLastError());
         if (!dev_io) {
-            if (x_out && n) CK(cudaMemcpyAsync(x_out, tx, sizeof(double) * (size_t)n, cudaMemcpyDeviceToHost, st));
-            if (y_out && m) CK(cudaMemcpyAsync(y_out, ty, sizeof(double) * (size_t)m, cudaMemcpyDeviceToHost, st));
+            if (x_out && n) CK(cudaMemcpyAsync(x_out, ox, sizeof(double) * (size_t)n, cudaMemcpyDeviceToHost, st));
+            if (y_out && m) CK(cudaMemcpyAsync(y_out, oy, sizeof(double) * (size_t)m, cudaMemcpyDeviceToHost, st));
         }
         Ctrl hc;
         CK(cudaMemcpyAsync(&hc, lp->ctl, sizeof(Ctrl), cudaMemcpyDeviceToHost, st));
@@ -1118,10 +1166,6 @@ static int solve_impl(uc_lp* lp, const uc_pdhg_params* pin, double* x_out, doubl
     } catch (const std::exception& e) {                        // nothing may unwind through the C ABI
         rc = fail(UC_ERR_NOMEM, std::string("uc_pdhg_solve: ") + e.what());
     }
-    if (tx0) cudaFree(tx0);
-    if (ty0) cudaFree(ty0);
-    if (tx) cudaFree(tx);
-    if (ty) cudaFree(ty);
     if (d_att) cudaFree(d_att);
     if (d_chk) cudaFree(d_chk);
     res->solve_seconds = now_s() - t_wall;
@@ -1354,6 +1398,8 @@ int uc_lp_get_scaling(uc_lp* lp, double* Dr_out, double* Dc_out) {
         }
     } catch (const CudaFail& f) {
         return fail(UC_ERR_CUDA, std::string(f.what) + ": " + cudaGetErrorString(f.e));
+    } catch (const std::exception& e) {                        // nothing may unwind through the C ABI
+        return fail(UC_ERR_NOMEM, e.what());
     }
     return UC_OK;
 }
@@ -1374,6 +1420,8 @@ int uc_lp_get_scaled_values(uc_lp* lp, int32_t from_transpose, double* val_out) 
         for (size_t k = 0; k < lsrc.size(); ++k) val_out[lsrc[k]] = t[k];
     } catch (const CudaFail& f) {
         return fail(UC_ERR_CUDA, std::string(f.what) + ": " + cudaGetErrorString(f.e));
+    } catch (const std::exception& e) {                        // nothing may unwind through the C ABI
+        return fail(UC_ERR_NOMEM, e.what());
     }
     return UC_OK;
 }

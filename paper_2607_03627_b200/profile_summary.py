@@ -44,6 +44,52 @@ def read_raw(report: str):
     return rows[0], rows[1], rows[2:]
 
 
+def sass_mix(report: str, kernel: str):
+    """Executed warp instructions by opcode for the first captured launch of `kernel` (ncu source page, SASS view) and
+    the number of pipeline steps it ran (= executed LDGDEPBAR, one cp.async.commit_group per step)."""
+    out = subprocess.run(["ncu", "-i", report, "--page", "source", "--csv", "--kernel-name", f"regex:{kernel}"],
+                         capture_output=True, text=True, check=True).stdout
+    rows = list(csv.reader(io.StringIO(out)))
+    heads = [i for i, r in enumerate(rows) if r and r[0] == "Address"]
+    if not heads:
+        return None
+    hdr = rows[heads[0]]
+    body = [r for r in rows[heads[0] + 1:(heads[1] - 1 if len(heads) > 1 else None)] if r and r[0].startswith("0x")]
+    ie, isrc = hdr.index("Instructions Executed"), hdr.index("Source")
+    mix, total = {}, 0
+    for r in body:
+        try:
+            e = int(r[ie])
+        except ValueError:
+            continue
+        w = r[isrc].split()
+        op = (w[1] if w[0].startswith("@") else w[0]).split(".")[0]
+        mix[op] = mix.get(op, 0) + e
+        total += e
+    return total, mix, len(body)
+
+
+def aggregate_launches(raw_csv: str, out_csv: str):
+    """Per-kernel aggregation of an `ncu --metrics gpu__time_duration.sum --csv` launch list: launches, mean and total
+    duration, share of the total (cold-cache, serialised launches: compare shares, not absolute times)."""
+    rows = [r for r in csv.reader(open(raw_csv)) if len(r) > 10]
+    hdr = rows[0]
+    ik, iv, iu, im = hdr.index("Kernel Name"), hdr.index("Metric Value"), hdr.index("Metric Unit"), hdr.index("Metric Name")
+    agg = {}
+    for r in rows[1:]:
+        if r[im] != "gpu__time_duration.sum":
+            continue
+        us = float(r[iv].replace(",", "")) * {"ns": 1e-3, "us": 1.0, "ms": 1e3}.get(r[iu], 1e-3)
+        a = agg.setdefault(r[ik].split("(")[0], [0, 0.0])
+        a[0] += 1; a[1] += us
+    total = sum(v[1] for v in agg.values()) or 1.0
+    with open(out_csv, "w") as f:
+        f.write("kernel,launches,mean_us,total_us,share_pct\n")
+        for k, (n, t) in sorted(agg.items(), key=lambda kv: -kv[1][1]):
+            f.write(f"{k},{n},{t / n:.2f},{t:.1f},{100 * t / total:.2f}\n")
+    return agg
+
+
 def to_bytes(value: str, unit: str) -> float:
     scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
     return float(value) * scale.get(unit, 1.0)
@@ -55,6 +101,8 @@ def main():
     ap.add_argument("--tag", required=True)
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--command", default="", help="the full command that produced the report (recorded in the summary)")
+    ap.add_argument("--launches", default="", help="raw `ncu --metrics gpu__time_duration.sum --csv` launch list to aggregate into profiles/<tag>_launches.csv")
+    ap.add_argument("--launches-command", default="")
     args = ap.parse_args()
     hdr, units, data = read_raw(args.report)
     col = {h: i for i, h in enumerate(hdr)}
@@ -89,7 +137,30 @@ def main():
             b = to_bytes(d[col["dram__bytes_read.sum"]], units[col["dram__bytes_read.sum"]]) + \
                 to_bytes(d[col["dram__bytes_write.sum"]], units[col["dram__bytes_write.sum"]])
             traffic.setdefault(kern, []).append(b)
+    lines += ["", "## Executed SASS of the first captured launch of each kernel (ncu source page, `--import-source on`)", "",
+              "A pipeline step = 32 rows x up to 4 entries (one `cp.async.commit_group`, SASS `LDGDEPBAR`, per step).", "",
+              "| kernel | static SASS instructions | warp instructions executed | steps | per step | asynchronous copies `LDGSTS` | plain loads `LDG` | stores `STG` | "
+              "TMA (`UBLKCP` / `UTMALDG`) | most executed opcodes per step |", "|---|---|---|---|---|---|---|---|---|---|"]
+    for kern in ("k_primal", "k_dual"):
+        m = sass_mix(args.report, kern)
+        if not m:
+            continue
+        total, mix, nstatic = m
+        steps = max(mix.get("LDGDEPBAR", 0), 1)
+        top = ", ".join(f"{op} {c / steps:.1f}" for op, c in sorted(mix.items(), key=lambda kv: -kv[1])[:12])
+        lines.append(f"| {kern} | {nstatic:,} | {total:,} | {steps:,} | {total / steps:.0f} | {mix.get('LDGSTS', 0):,} | {mix.get('LDG', 0):,} | "
+                     f"{mix.get('STG', 0):,} | {mix.get('UBLKCP', 0) + mix.get('UTMALDG', 0)} | {top} |")
     os.makedirs(os.path.join(ROOT, "profiles"), exist_ok=True)
+    if args.launches:
+        agg = aggregate_launches(args.launches, os.path.join(ROOT, "profiles", f"{args.tag}_launches.csv"))
+        total = sum(v[1] for v in agg.values()) or 1.0
+        lines += ["", f"## Launch list (`profiles/{args.tag}_launches.csv`)", ""]
+        if args.launches_command:
+            lines += ["```", args.launches_command, "```", ""]
+        lines += ["Cold-cache, serialised launches: the SHARE of a kernel is what compares with the un-profiled run, not its absolute time.", "",
+                  "| kernel | launches | mean us | share of the kernel time |", "|---|---|---|---|"]
+        for k, (n, t) in sorted(agg.items(), key=lambda kv: -kv[1][1]):
+            lines.append(f"| {k} | {n} | {t / n:.2f} | {100 * t / total:.2f} % |")
     with open(os.path.join(ROOT, "profiles", f"{args.tag}_summary.md"), "w") as f:
         f.write("\n".join(lines) + "\n")
     tpath = os.path.join(ROOT, "profiles", "r02_traffic.json")
