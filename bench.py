@@ -199,22 +199,24 @@ def all_configs_table(batch_sizes=(1, 4, 16, 45)):
         h.close()
         del lp, x, y
     print()
-    print("| workload | LPs in one uc_pdhg_solve_batch call (16 in flight) | aggregate attempts/s | per-LP attempts/s | results identical to a solo solve |")
-    print("|---|---|---|---|---|")
-    for name, key in (("UC config 0", 0), ("UC tuned-presolve shape", "tuned_presolve"), ("UC config 1", 1)):
+    print("| workload | CTAs per kernel (max_ctas) | LPs in one uc_pdhg_solve_batch call (16 in flight) | aggregate attempts/s | per-LP attempts/s | results identical to a solo solve |")
+    print("|---|---|---|---|---|---|")
+    for name, key, limits in (("UC config 0", 0, (0,)), ("UC tuned-presolve shape", "tuned_presolve", (0, 37, 18)), ("UC config 1", 1, (0, 37))):
         lp = uc_config(key)
         F = 2048
-        hs = [P.UcLp(lp, device=0) for _ in range(max(batch_sizes))]
-        solo = hs[0].solve(fixed_iterations=F)
-        for nb in batch_sizes:
-            for _ in range(2):
-                torch.cuda.synchronize(); t = time.perf_counter()
-                out = P.solve_batch(hs[:nb], fixed_iterations=F)
-                dt = time.perf_counter() - t
-            same = all(np.array_equal(o.x, solo.x) and np.array_equal(o.y, solo.y) for o in out)
-            print(f"| {name} | {nb} | {nb * F / dt:.0f} | {F / dt:.0f} | {same} |", flush=True)
-        for h in hs:
-            h.close()
+        with P.UcLp(lp, device=0) as h0:
+            solo = h0.solve(fixed_iterations=F)
+        for lim in limits:
+            hs = [P.UcLp(lp, device=0, max_ctas=lim) for _ in range(max(batch_sizes))]
+            for nb in batch_sizes:
+                for _ in range(2):
+                    torch.cuda.synchronize(); t = time.perf_counter()
+                    out = P.solve_batch(hs[:nb], fixed_iterations=F)
+                    dt = time.perf_counter() - t
+                same = all(np.array_equal(o.x, solo.x) and np.array_equal(o.y, solo.y) for o in out)
+                print(f"| {name} | {'all SMs' if lim == 0 else lim} | {nb} | {nb * F / dt:.0f} | {F / dt:.0f} | {same} |", flush=True)
+            for h in hs:
+                h.close()
 
 
 def main():

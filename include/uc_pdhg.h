@@ -67,6 +67,10 @@ typedef struct {
     int32_t host_ingest;        /* 0 (default): step A1 -- permutations, explicit transpose, both layouts -- runs as kernels on
                                    the device from one copy of the caller's CSR; 1: the host builders (the checker's code)
                                    build them and upload.  Both give the same layouts bit for bit (uc_lp_compare_layout) */
+    int32_t max_ctas;           /* 0 (default): the kernels of this handle may use every SM.  > 0: at most this many CTAs per
+                                   kernel -- for LPs solved SIDE BY SIDE (uc_pdhg_solve_batch, the paper's 45 scenarios): a
+                                   mid-size LP spread over all SMs has one slice per warp and leaves no SM to its neighbours;
+                                   with a quarter of the SMs each, four of them run at once.  Results do not depend on it */
 } uc_lp_options;
 
 void uc_lp_default_options(uc_lp_options* opt);

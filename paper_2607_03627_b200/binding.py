@@ -22,7 +22,7 @@ class UcError(RuntimeError):
 class Options(C.Structure):
     _fields_ = [("device", C.c_int32), ("ruiz_iters", C.c_int32), ("pc_alpha", C.c_double),
                 ("sell_window", C.c_int32), ("long_row_threshold", C.c_int32),
-                ("keep_source_map", C.c_int32), ("index_compression", C.c_int32), ("host_ingest", C.c_int32)]
+                ("keep_source_map", C.c_int32), ("index_compression", C.c_int32), ("host_ingest", C.c_int32), ("max_ctas", C.c_int32)]
 
 
 class Params(C.Structure):

@@ -684,7 +684,7 @@ double uc_host_exp_rounded(double x) { return exp_rounded(x); }
 void uc_lp_default_options(uc_lp_options* o) {
     if (!o) return;
     o->device = -1; o->ruiz_iters = 10; o->pc_alpha = 1.0; o->sell_window = 4096; o->long_row_threshold = 32;
-    o->keep_source_map = 0; o->index_compression = 1; o->host_ingest = 0;
+    o->keep_source_map = 0; o->index_compression = 1; o->host_ingest = 0; o->max_ctas = 0;
 }
 
 void uc_pdhg_default_params(uc_pdhg_params* p) {
@@ -705,7 +705,7 @@ int uc_lp_create(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, cons
     uc_lp_options opt;
     uc_lp_default_options(&opt);
     if (opt_in) opt = *opt_in;
-    if (opt.ruiz_iters < 0 || opt.pc_alpha < 0.0 || opt.pc_alpha > 2.0 || opt.sell_window < 32 || opt.long_row_threshold < 1)
+    if (opt.ruiz_iters < 0 || opt.pc_alpha < 0.0 || opt.pc_alpha > 2.0 || opt.sell_window < 32 || opt.long_row_threshold < 1 || opt.max_ctas < 0)
         return fail(UC_ERR_INVALID, "bad uc_lp_options");
     const bool tim = std::getenv("UC_CREATE_TIMING") != nullptr;
     double tph = now_s();
@@ -747,7 +747,9 @@ int uc_lp_create(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, cons
         // persistent grids of the attempt kernels: kCtasPerSm CTAs per SM, never more CTAs than work, and no more
         // consumer warps per CTA than the slices need (at least kMinWarps, at most the compiled maximum)
         auto attempt_shape = [&](int64_t nshort, int64_t nlong, int max_warps, int& grid, int& warps) {
-            const int64_t cap = (int64_t)kCtasPerSm * std::max(sms, 1), slices = (nshort + 31) / 32;
+            int64_t cap = (int64_t)kCtasPerSm * std::max(sms, 1);
+            if (opt.max_ctas > 0) cap = std::min<int64_t>(cap, opt.max_ctas);
+            const int64_t slices = (nshort + 31) / 32;
             warps = (int)std::max<int64_t>(std::min<int64_t>(kMinWarps, max_warps), std::min<int64_t>(max_warps, (slices + cap - 1) / cap));
             grid = (int)std::max<int64_t>(1, std::min<int64_t>(cap, std::max<int64_t>((slices + warps - 1) / warps, nlong)));
         };
@@ -899,7 +901,7 @@ int uc_lp_create(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, cons
         {   // check kernels: persistent blocks, kCheckMinBlocks per SM, grid-stride over the layout's 256-row blocks
             int sms = 0;
             CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-            const int cap = kCheckMinBlocks * std::max(sms, 1);
+            const int cap = kCheckMinBlocks * std::max(opt.max_ctas > 0 ? std::min(sms, opt.max_ctas) : sms, 1);
             V.gridA = std::max(1, std::min(cap, lp->KT.grid)); V.gridB = std::max(1, std::min(cap, lp->K.grid));
         }
         V.gridPA = gridPA; V.gridPB = gridPB;

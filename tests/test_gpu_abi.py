@@ -150,3 +150,19 @@ def test_solve_batch_results_are_those_of_solo_solves(lp1):
     finally:
         for h in handles:
             h.close()
+
+
+def test_results_do_not_depend_on_the_cta_limit(lp1):
+    """uc_lp_options.max_ctas only changes how the slices are dealt to CTAs and warps: bit-identical iterates."""
+    with P.UcLp(lp1) as a, P.UcLp(lp1, max_ctas=5) as b, P.UcLp(lp1, max_ctas=37) as c:
+        sa, sb, sc = (h.solve(fixed_iterations=256, trace_attempts=256) for h in (a, b, c))
+    for s in (sb, sc):
+        np.testing.assert_array_equal(s.x, sa.x); np.testing.assert_array_equal(s.y, sa.y)
+        np.testing.assert_array_equal(s.attempts["eta_used"], sa.attempts["eta_used"])
+
+
+def test_timeline_hook_is_refused_by_the_product_build(lp1):
+    with P.UcLp(lp1) as h:
+        with pytest.raises(P.UcError) as e:
+            h.timeline(4)
+    assert "UC_TIMELINE" in str(e.value)
