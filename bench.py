@@ -219,6 +219,27 @@ def all_configs_table(batch_sizes=(1, 4, 16, 45)):
                 h.close()
 
 
+def sweep_line(args):
+    """One size of the roofline sweep (BASELINE.json configs[4]): attempts/s and effective bandwidth of 200 fixed attempts."""
+    import torch
+    import paper_2607_03627_b200 as P
+    from workloads import sweep_config
+    lp = sweep_config(args.sweep_seed)
+    peak, _ = load_peaks()
+    st = torch.cuda.Stream()
+    with P.UcLp(lp, device=0) as h:
+        x = torch.empty(lp.n, dtype=torch.float64, device="cuda"); y = torch.empty(lp.m, dtype=torch.float64, device="cuda")
+        for _ in range(max(args.warmup, 1)):
+            r = h.solve_device(x, y, fixed_iterations=200, stream=st.cuda_stream)
+        loop = 0.0
+        for _ in range(max(args.steps, 1)):
+            loop += h.solve_device(x, y, fixed_iterations=200, stream=st.cuda_stream).loop_seconds
+        bp, bd = algorithmic_bytes(lp.m, lp.n, lp.nnz, h.info())
+    us = loop * 1e6 / (200 * max(args.steps, 1))
+    print(json.dumps({"metric": METRIC, "value": 1e6 / us, "unit": UNIT, "config": {"workload": f"BASELINE.json configs[4] seed {args.sweep_seed}: random LP (m={lp.m}, n={lp.n}, nnz={lp.nnz}), 200 fixed attempts"},
+                      "us_per_attempt": us, "algorithmic_bytes": {"k_primal": bp, "k_dual": bd}, "GB/s": (bp + bd) / us / 1e3, "frac_of_peak": (bp + bd) / us / 1e3 / peak}), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -232,9 +253,13 @@ def main():
     ap.add_argument("--clock-sample-ms", type=int, default=100)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--all-configs", action="store_true", help="print the table over all configs instead of the bench line")
+    ap.add_argument("--sweep-seed", type=int, default=None, help="run BASELINE.json configs[4] (roofline sweep, seeds 10-14) instead: "
+                    "--steps calls of 200 fixed attempts, a short line without e2e (what the ncu DRAM-byte captures of profiles/ run)")
     args = ap.parse_args()
     if args.all_configs:
         return all_configs_table()
+    if args.sweep_seed is not None:
+        return sweep_line(args)
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
     rank = int(os.environ.get("RANK", "0"))
