@@ -6,33 +6,37 @@
 //                          dy.(K~ dx) ; the last CTA finishes the three reductions and runs the
 //                          step-size rule and the accept test                              (R3..R5)
 //
-// Both are HBM-bound streams (0.16 flop/B) of rows with ~3.4 entries, each entry needing an irregular
-// 8/16-byte gather.  The design question is how to keep ~50 KB per SM in flight AND issue ~45k gathers per
-// SM per kernel.  What was measured on B200 (profiles/):
+// Both stream rows with ~3.4 entries (0.16 flop/B), each entry needing an irregular 8/16-byte gather.  What bounds them
+// is not DRAM and not instruction issue but the path between L2 and the SMs: every gather that misses L1 is its own L2
+// request for a 32-byte sector (profiles/r02a: 5,900 B/cycle of L2 sectors chip-wide against a ~6,300 B/cycle ceiling,
+// DRAM at 42-54 %; 17 % fewer instructions changed nothing).  What was measured on B200 (profiles/):
 //   * a 1-D TMA bulk copy (cp.async.bulk) costs its issuing thread ~160 cycles whatever its size -- right for
-//     16 KB tiles, hopeless for the 2 KB vector segments and ~1 KB index/value chunks this path is made of;
+//     16 KB tiles, hopeless for the 2 KB vector segments and ~1 KB value chunks this path is made of;
 //   * a coalesced cp.async (LDGSTS.128) costs ~8 cycles and holds no register while in flight;
-//   * divergent gathers run at ~1000 gathers/us/SM from 4 issuing warps but ~1500 from 8 or more.
-// Hence: persistent CTAs (one per SM) of kAttWarps CONSUMER warps, every one of which runs its own
-// three-stage software pipeline on its own shared-memory rings, with NO block-level synchronisation inside
-// the loop.  The unit of work is a STEP (uc_format.hpp): up to kChunkT entries per row of one slice (32 rows,
-// one per lane).  For its step j a warp has, in flight at the same time,
-//     A(j + kDA): cp.async of the step's column indices                         -> index ring
-//     B(j + kDB): cp.async of the step's matrix values, of the 32-row segments of the per-row vectors
-//                 (last step of a slice only) and, using the indices that A brought in, one 8/16-byte
-//                 cp.async per stored entry e:  gv[e] <- src[col[e]]  (the entry of y, or of the pair
-//                 {xbar, dx}, that e multiplies)                                -> data ring
-//     C(j):       everything read from shared memory: row sums left to right, update, coalesced stores.
-// One cp.async group is committed per step; cp.async.wait_group kDB + __syncwarp is the only wait.  A slice
-// wider than kChunkT is a run of consecutive steps whose row sums stay in registers.  The schedule (each slice
-// to the least-loaded warp, built at create time) is static, so results are reproducible bit for bit.  One extra warp
-// per CTA takes the rows longer than the sliced-ELL threshold (the T reserve rows of the UC LP), one row at a
-// time, concurrently.
-// L2 policy: streamed-once data is loaded (cp.async.cg, L1 bypass) and stored evict_first; the gathered vectors
-// (y', {xbar, dx}) are stored evict_last so that the gathers of the NEXT kernel hit in the 126 MB L2.
-// Every thread keeps its double-double partial sums in registers across all its steps; there is ONE block
-// reduction per kernel, then one partial per CTA; warp 0 of the last CTA to finish (ticket) adds the <= #SM
-// partials with shuffles only and runs the step rule on scalars it fetched while the kernel started.
+//   * an asynchronous copy whose shared-memory destination is not aligned like its global source fetches every global
+//     sector twice (hence the 128-byte data slots);
+//   * a gather that allocates in L1 (cp.async.ca) pays off once a CTA sweeps a CONTIGUOUS range of rows: neighbouring
+//     rows gather from the same few blocks of the vector (uc_format.hpp build_schedule).
+// Hence: persistent CTAs (one per SM) of up to 15 CONSUMER warps, every one of which runs its own three-stage software
+// pipeline on its own shared-memory data slots, with NO block-level synchronisation inside the loop.  The unit of work
+// is a STEP (uc_format.hpp): up to kChunkT entries per row of one slice (32 rows, one per lane).  In the iteration
+// that computes step j a warp also issues
+//     A(j + DB + 2): plain loads of the step's column indices into REGISTERS (2 or 4 bytes per lane and entry)
+//     B(j + DB):     cp.async of the step's matrix values, of the 32-row segments of the per-row vectors (last step of a
+//                    slice only) and, with the indices A brought in, one 8/16-byte cp.async per stored entry e:
+//                    gv[e] <- src[col[e]]  (the entry of y, or of the pair {xbar, dx}, that e multiplies)  -> data slots
+//     C(j):          everything read from shared memory: row sums left to right, update, coalesced stores.
+// One cp.async group is committed per step; cp.async.wait_group DB + __syncwarp is the only wait.  A slice wider than
+// kChunkT is a run of consecutive steps whose row sums stay in registers.  The schedule (a contiguous range of slices
+// per CTA, dealt inside the CTA to the least-loaded warp, built at create time) is static, so a solve is reproducible bit
+// for bit.  One extra warp per CTA takes the rows longer than the sliced-ELL threshold (the T reserve rows of the UC
+// LP), one row at a time, concurrently.
+// L2 policy: streamed-once data is loaded (cp.async.cg / ld.global.nc.L1::no_allocate) and stored evict_first; the
+// gathered vectors (y', {xbar, dx}) are stored evict_last so that the gathers of the NEXT kernel hit in the 126 MB L2.
+// Every thread keeps its double-double partial sums in registers across all its steps; there is ONE block reduction
+// per kernel, then one partial per CTA; warp 0 of the last CTA to finish (ticket) adds the <= #SM partials with
+// shuffles only and runs the step rule on scalars parked in shared memory while the kernel started (the serial tail
+// of every attempt: DESIGN.md section 7, profiles/r02c_timeline.md).
 //
 // Arithmetic is unchanged from the sequential statement: row sums left to right in CSR order, multiply
 // and add rounded separately (-fmad=false), long reductions in double-double (order-independent once
@@ -64,8 +68,8 @@ namespace ucpdhg {
 constexpr int kPrimalWarps = UC_PRIMAL_WARPS, kDualWarps = UC_DUAL_WARPS, kMinWarps = UC_MIN_WARPS;
 constexpr int kCtasPerSm = UC_CTAS_PER_SM;
 constexpr int kPrimalThreads = (kPrimalWarps + 1) * 32, kDualThreads = (kDualWarps + 1) * 32;   // + long-row warp
-// pipeline depth, per kernel: data (values, vectors, gathers) run kDB steps ahead of the compute, indices
-// kDA = 2 kDB + 1 steps ahead (a group is complete kDB commits later); kDB + 2 index slots, kDB + 1 data slots
+// pipeline depth, per kernel: the data copies (values, vectors, gathers) run DB steps ahead of the compute (DB + 1 data
+// slots; 1 or 3), the index loads DB + 2 steps ahead.  DB = 3 was measured slower: it takes the L1 the gathers live on.
 #ifndef UC_PRIMAL_DB
 #define UC_PRIMAL_DB UC_DB
 #endif

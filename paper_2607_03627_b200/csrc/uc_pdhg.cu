@@ -28,6 +28,7 @@ thread_local std::string g_err;
 int fail(int code, const std::string& msg) { g_err = msg; return code; }
 
 struct CudaFail { cudaError_t e; const char* what; };
+struct TooLarge { const char* what; };                            // a size limit of the layout, not an allocation failure
 #define CK(call)                                                 \
     do {                                                         \
         cudaError_t e__ = (call);                                \
@@ -275,7 +276,7 @@ Sell device_side(uc_lp* lp, TempArena& T, const FillSrc& S, const int* len, long
     }
     k_ing_close_scan<<<1, 32, 0, st>>>(lptr, llen, nlong);
     const long long nslots = d2h_ll(sp + nslices, st), lnnz = d2h_ll(lptr + nlong, st);
-    if (nslots >= (1LL << 31)) throw std::bad_alloc();              // step descriptors address entries / 32 in 26 bits
+    if (nslots >= (1LL << 31)) throw TooLarge{"more than 2^31 stored slots in one sliced-ELL layout (step descriptors address entries / 32 in 26 bits)"};
     stats.slots = nslots; stats.long_nnz = lnnz;
     // arrays (zeroed by dalloc: padding slots are (col 0, val 0.0))
     int* col = lp->dalloc<int>((size_t)nslots);
@@ -350,10 +351,8 @@ double reduce_to_host(uc_lp* lp, const double* v, long long count, int op, dd* p
 }
 
 // R1: Ruiz x ruiz_iters, then Pock-Chambolle(alpha); accumulates Dr, Dc; scales both layouts.
-void precondition(uc_lp* lp, cudaStream_t st) {
+void precondition(uc_lp* lp, cudaStream_t st, double* r, double* s) {      // r[m], s[n]: scratch of the caller
     const long long m = lp->m, n = lp->n;
-    double* r = lp->dalloc<double>((size_t)m);
-    double* s = lp->dalloc<double>((size_t)n);
     k_vec_fill<<<cdiv(std::max<long long>(m, 1), 256), 256, 0, st>>>(lp->Dr, 1.0, m);
     k_vec_fill<<<cdiv(std::max<long long>(n, 1), 256), 256, 0, st>>>(lp->Dc, 1.0, n);
     const double alpha = lp->opt.pc_alpha;
@@ -762,7 +761,7 @@ int uc_lp_create(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, cons
         // everything the ingest kernels and sorts need
         TempArena T;
         {
-            const size_t vec_bytes = (size_t)8 * (size_t)(m + 3 * n) + (size_t)m + 8 * 512 + sizeof(dd) * 1024 + 4096;
+            const size_t vec_bytes = (size_t)8 * (size_t)(2 * m + 4 * n) + (size_t)m + 12 * 512 + sizeof(dd) * 1024 + 4096;
             const size_t src_bytes = want_src ? 16 * ((size_t)nnz + 32 * (size_t)(m + n) / 32 + 1024) * 3 : 0;
             const size_t ingest_bytes = opt.host_ingest ? 0 : (size_t)(8 * (m + 1) + 44 * nnz + 28 * n + 4 * m + 44 * (m + n)) +
                                         ((size_t)(m + n) / 32 + 2) * 40 + src_bytes + 256 * 64 + ((size_t)64 << 20);
@@ -773,6 +772,7 @@ int uc_lp_create(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, cons
         double* dl = TV.get<double>((size_t)n + 1); double* du = TV.get<double>((size_t)n + 1);
         char* dsense = TV.get<char>((size_t)m + 1);
         dd* part = TV.get<dd>(1024); double* scal = TV.get<double>(8);
+        double* rscr = TV.get<double>((size_t)m + 1); double* sscr = TV.get<double>((size_t)n + 1);      // Ruiz / Pock-Chambolle factors of a pass
         cudaError_t vec_err = cudaSuccess;
         std::thread vec_up([&] {
             cudaSetDevice(dev);
@@ -856,7 +856,7 @@ int uc_lp_create(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, cons
             try {
                 cudaSetDevice(dev);
                 build_K(row_ptr, col_idx, val, want_src, P);
-                if (P.K.col.size() >= (size_t)1 << 31) throw std::bad_alloc();   // step descriptors address entries / 32 in 26 bits
+                if (P.K.col.size() >= (size_t)1 << 31) throw TooLarge{"more than 2^31 stored slots in one sliced-ELL layout"};
                 compress_columns(P.K, opt.index_compression != 0);
                 build_schedule(P.K, gridPB, warpsPB);
                 lp->K = upload_sell(lp, P.K);
@@ -865,7 +865,7 @@ int uc_lp_create(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, cons
         try {
             build_KT(row_ptr, col_idx, val, want_src, P);
             phase("build_KT");
-            if (P.KT.col.size() >= (size_t)1 << 31) throw std::bad_alloc();
+            if (P.KT.col.size() >= (size_t)1 << 31) throw TooLarge{"more than 2^31 stored slots in one sliced-ELL layout"};
             compress_columns(P.KT, opt.index_compression != 0);
             phase("compress KT");
             build_schedule(P.KT, gridPA, warpsPA);
@@ -931,7 +931,7 @@ int uc_lp_create(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, cons
         reduce_to_dev(db, m, 0, part, scal + 0, st);
         reduce_to_dev(dc, n, 0, part, scal + 1, st);
         CK(cudaEventRecord(lp->ev_t0, st));
-        precondition(lp, st);
+        precondition(lp, st, rscr, sscr);
         k_scale_problem<<<V.gridR, kBlock, 0, st>>>(n, m, db, dc, dl, du, dsense, lp->perm_c, lp->perm_r, lp->Dr, lp->Dc,
                                                     lp->qs, lp->cs, lp->ls, lp->us, lp->isG);
         CK(cudaGetLastError());
@@ -958,6 +958,10 @@ int uc_lp_create(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, cons
         join_validation();
         destroy_impl(lp);
         return fail(code, msg);
+    } catch (const TooLarge& t) {
+        join_validation();
+        destroy_impl(lp);
+        return fail(UC_ERR_INVALID, t.what);
     } catch (const std::bad_alloc&) {
         join_validation();
         destroy_impl(lp);
