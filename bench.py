@@ -314,6 +314,9 @@ def main():
     seconds = e0.elapsed_time(e1) * 1e-3
     # dominant kernel, timed live with CUDA events on the launching stream
     primal_ms, dual_ms = h.time_kernels(64, stream=stream.cuda_stream)
+    # the same attempts with ONE check at the end instead of one per 64: what the two attempt kernels take inside the
+    # graph, under programmatic dependent launch, without the event records that separate them in time_kernels
+    nocheck_s = h.solve_device(x, y, fixed_iterations=A, check_every=A, stream=stream.cuda_stream).loop_seconds
     clocks = sampler.stop()
     tmax, units = aggregate(seconds, args.steps * A, dist, dev)
 
@@ -334,6 +337,13 @@ def main():
                 "frac_dram": (tr / (dom[2] * 1e-3) / 1e9 / peak) if tr else None,
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": dom[1], "kernel_ms": dom[2],
                 "other_kernel": {"k_primal_ms": primal_ms, "k_dual_ms": dual_ms, "k_primal_bytes": bp, "k_dual_bytes": bd},
+                "in_graph": {"what": "context for kernel_ms: an event record between two kernels keeps the next one from starting early "
+                                     "(programmatic dependent launch), so the per-kernel event times add up to more than an attempt takes in "
+                                     "the graph; pair_ms = both kernels per attempt inside the graph (a run with one check per "
+                                     f"{A} attempts), split by the ratio of the event times",
+                             "pair_ms": 1e3 * nocheck_s / A, "checks_ms_per_attempt": att_ms - 1e3 * nocheck_s / A,
+                             "k_primal_ms_est": 1e3 * nocheck_s / A * primal_ms / (primal_ms + dual_ms),
+                             "k_dual_ms_est": 1e3 * nocheck_s / A * dual_ms / (primal_ms + dual_ms)},
                 "attempt": {"algorithmic_bytes": bp + bd, "algorithmic_bytes_32bit_indices": sp + sd, "ms_in_graph": att_ms,
                             "GB/s": (bp + bd) / (att_ms * 1e-3) / 1e9,
                             "frac_of_peak": (bp + bd) / (att_ms * 1e-3) / 1e9 / peak,
