@@ -232,6 +232,39 @@ int uc_lp_get_scaled_values(uc_lp* lp, int32_t from_transpose, double* val_out);
    tests/test_gpu_parity.py, which runs k_primal + k_dual once from a warm start through uc_pdhg_solve.) */
 int uc_lp_spmv(uc_lp* lp, int32_t transpose, const double* v, double* out);
 
+/* uc_lp_spmv for callers that must not allocate device memory.
+ *
+ * Who that is: code that runs beside latency-critical work on the same GPU (cudaMalloc and cudaFree synchronise the
+ * whole device, so one call stalls every other stream -- a racing PDHG solve, included); code inside a
+ * process whose device memory has all been handed to a pool or to another library's caching allocator, where a raw
+ * cudaMalloc fails although memory is "free"; and code under a no-allocation rule after start-up (fixed memory budget,
+ * certified or long-running services that must not fragment or grow).  uc_lp_spmv allocates four temporary vectors per
+ * call; this entry point allocates nothing and calls no cudaMalloc, cudaFree or other allocating routine.
+ *
+ * It computes the same product with the same kernels, so the result equals uc_lp_spmv's bit for bit:
+ *   out = Ktilde v (transpose = 0; v[n], out[m])  or  Ktilde' v (transpose = 1; v[m], out[n]),  original order.
+ * v_device / out_device are DEVICE pointers on the handle's device, owned by the caller; they must not overlap.  The two
+ * intermediate vectors (v and the product in the layout's own order) live in ONE fixed array inside the library, 2 MiB
+ * on every GPU that has loaded it, held until the process exits.
+ *
+ * Limit: round m and n up to multiples of 32; their sum must not exceed UC_SPMV_STATIC_MAX_DOUBLES (262,144 -- config 0
+ * and config 1 of BASELINE.json fit, the larger ones do not).  A larger handle gets UC_ERR_INVALID and a message naming
+ * the limit; nothing is launched.  Other errors as uc_lp_spmv (UC_ERR_BUSY while a solve runs on the handle).
+ *
+ * Stream order: the three kernels are enqueued on `stream` (cudaStream_t; NULL = the handle's own stream) and the call
+ * returns without waiting; out_device is complete when the stream reaches that point.
+ *
+ * Sharing: the array is one per GPU, shared by every handle, stream and host thread, and it keeps whatever the last call
+ * wrote.  Nothing in it needs to start at zero (every entry that is read has been written earlier in the same call), so
+ * back-to-back calls on ONE stream are safe.  Two calls that can overlap on the GPU -- different streams, or different
+ * threads using different streams -- race on it and both results are garbage: order them yourself (one stream, or an
+ * event between them).
+ *
+ * First call on a device: it looks up the array's device address (cudaGetSymbolAddress, with the handle's device made
+ * current) and remembers it per device.  Make that first call during set-up, before any stream capture is begun. */
+#define UC_SPMV_STATIC_MAX_DOUBLES 262144
+int uc_lp_spmv_static(uc_lp* lp, int32_t transpose, const double* v_device, double* out_device, void* stream);
+
 /* Host-only self-check of ingest step A1 (no GPU needed): builds the row / column permutations, the explicit
    transpose, both SELL-32 layouts and both attempt schedules (for `sched_ctas` CTAs of `warps_per_cta` consumer warps)
    exactly as uc_lp_create does, and verifies them entry by entry against the caller's CSR: stored entries are the

@@ -59,9 +59,11 @@ ATTEMPT_DTYPE = np.dtype([("eta_used", "f8"), ("eta_bar", "f8"), ("eta_next", "f
 CHECK_DTYPE = np.dtype([("k", "i8"), ("restart_kind", "i4"), ("candidate", "i4"), ("omega_after", "f8"),
                         ("mu_c", "f8"), ("mu_r", "f8"), ("relkkt_cur", "f8"), ("relkkt_avg", "f8")])
 
+SPMV_STATIC_MAX_DOUBLES = 262144      # UC_SPMV_STATIC_MAX_DOUBLES of include/uc_pdhg.h
+
 EXPORTS = ["uc_lp_default_options", "uc_lp_create", "uc_lp_update_bounds", "uc_lp_update_objective", "uc_lp_destroy",
            "uc_pdhg_default_params", "uc_pdhg_solve", "uc_pdhg_solve_device", "uc_pdhg_solve_batch", "uc_pdhg_cancel", "uc_pdhg_time_kernels", "uc_pdhg_timeline", "uc_lp_compare_layout",
-           "uc_lp_get_info", "uc_lp_get_scaling", "uc_lp_get_scaled_values", "uc_lp_spmv", "uc_last_error",
+           "uc_lp_get_info", "uc_lp_get_scaling", "uc_lp_get_scaled_values", "uc_lp_spmv", "uc_lp_spmv_static", "uc_last_error",
            "uc_host_log_rounded", "uc_host_exp_rounded", "uc_host_layout_selftest"]
 
 _lib = None
@@ -105,6 +107,7 @@ def load_library(build_if_missing: bool = True):
     lib.uc_lp_get_scaling.argtypes = [C.c_void_p] * 3
     lib.uc_lp_get_scaled_values.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
     lib.uc_lp_spmv.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
+    lib.uc_lp_spmv_static.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
     _lib = lib
     return lib
 
@@ -297,6 +300,14 @@ class UcLp:
         out = np.zeros(max(nout, 1))
         _check(self.lib.uc_lp_spmv(self._h, int(bool(transpose)), vp, C.c_void_p(out.ctypes.data)))
         return out[:nout]
+
+    def spmv_static(self, v_device_ptr, out_device_ptr, transpose=False, stream=None) -> None:
+        """uc_lp_spmv_static: the product of `spmv` for callers that must not allocate device memory (the intermediates
+        sit in a fixed 2 MiB array inside the library; m + n is limited to SPMV_STATIC_MAX_DOUBLES).  Both arguments are
+        device addresses (ints) of caller-owned float64 buffers on the handle's device; the kernels are enqueued on
+        `stream` (None = the handle's stream) and the call does not wait for them.  See include/uc_pdhg.h."""
+        _check(self.lib.uc_lp_spmv_static(self._h, int(bool(transpose)), C.c_void_p(int(v_device_ptr)), C.c_void_p(int(out_device_ptr)),
+                                          C.c_void_p(int(stream)) if stream is not None else None))
 
     def solve(self, x0=None, y0=None, trace_attempts=0, trace_checks=0, want_xy=True, stream=None, **params) -> Solution:
         """uc_pdhg_solve: host buffers in and out (H2D / D2H inside the call)."""

@@ -1468,3 +1468,74 @@ int uc_lp_spmv(uc_lp* lp, int32_t transpose, const double* v, double* out) {
 }
 
 }  // extern "C"
+
+// --------------------------------------------------------------------------------- uc_lp_spmv_static (include/uc_pdhg.h)
+// The same three kernels as uc_lp_spmv (k_gather -> k_spmv -> k_scatter), for callers that may not allocate device memory:
+// the permuted input and the permuted result, which uc_lp_spmv puts into two cudaMalloc'ed buffers, live in this fixed
+// array instead.  It is part of the library image: every device that loads libuc_pdhg.so holds these
+// UC_SPMV_STATIC_MAX_DOUBLES * 8 bytes (2 MiB) until the process exits, whether the entry point is ever called or not.
+// One array per device, shared by every handle, stream and thread: see the header for what that means for callers.
+static __device__ __align__(256) double g_spmv_static_scratch[UC_SPMV_STATIC_MAX_DOUBLES];
+
+namespace {
+
+constexpr int kStaticMaxDevices = 64;
+std::mutex g_spmv_static_mu;
+double* g_spmv_static_addr[kStaticMaxDevices] = {};   // device address of the array, per device; nullptr = not looked up yet
+
+// In host code `g_spmv_static_scratch` is only the host-side shadow of the symbol: its address means nothing to a kernel.
+// The device address is asked for once per device, with that device current (the array exists once per device).
+// Returns cudaSuccess and the address, or the error of the lookup (nothing is cached then: the next call tries again).
+cudaError_t spmv_static_scratch(int device, double** out) {
+    std::lock_guard<std::mutex> g(g_spmv_static_mu);
+    if (!g_spmv_static_addr[device]) {
+        void* p = nullptr;
+        cudaError_t e = cudaGetSymbolAddress(&p, g_spmv_static_scratch);
+        if (e != cudaSuccess) return e;
+        g_spmv_static_addr[device] = (double*)p;
+    }
+    *out = g_spmv_static_addr[device];
+    return cudaSuccess;
+}
+
+}  // namespace
+
+extern "C" int uc_lp_spmv_static(uc_lp* lp, int32_t transpose, const double* v_device, double* out_device, void* stream) {
+    if (!lp) return fail(UC_ERR_INVALID, "handle is NULL");
+    const long long nin = transpose ? lp->m : lp->n, nout = transpose ? lp->n : lp->m;
+    if ((nin > 0 && !v_device) || (nout > 0 && !out_device)) return fail(UC_ERR_INVALID, "NULL argument");
+    // each of the two scratch vectors starts on a 256-byte boundary of the array
+    const long long nin_pad = (nin + 31) / 32 * 32, nout_pad = (nout + 31) / 32 * 32;
+    if (nin_pad + nout_pad > (long long)UC_SPMV_STATIC_MAX_DOUBLES)
+        return fail(UC_ERR_INVALID, "uc_lp_spmv_static: m + n = " + std::to_string(nin + nout) + " (each rounded up to a multiple of 32) exceeds the "
+                    "fixed scratch of UC_SPMV_STATIC_MAX_DOUBLES = " + std::to_string((long long)UC_SPMV_STATIC_MAX_DOUBLES) +
+                    " doubles; use uc_lp_spmv, which allocates what it needs");
+    if (lp->device < 0 || lp->device >= kStaticMaxDevices) return fail(UC_ERR_INVALID, "uc_lp_spmv_static: device ordinal above 63");
+    int expected = 0;
+    if (!lp->busy.compare_exchange_strong(expected, 1)) return fail(UC_ERR_BUSY, "a solve is running on this handle");
+    int rc = UC_OK;
+    {
+        DeviceGuard guard(lp->device);
+        double* scratch = nullptr;
+        cudaError_t e = spmv_static_scratch(lp->device, &scratch);
+        if (e != cudaSuccess) rc = fail(UC_ERR_CUDA, std::string("cudaGetSymbolAddress(g_spmv_static_scratch): ") + cudaGetErrorString(e));
+        else {
+            const long long* pin = transpose ? lp->perm_r : lp->perm_c;
+            const long long* pout = transpose ? lp->perm_c : lp->perm_r;
+            const Sell& S = transpose ? lp->KT : lp->K;
+            cudaStream_t st = stream ? (cudaStream_t)stream : lp->own_stream;
+            double* dperm = scratch;               // v in the layout's column order, nin entries
+            double* dres = scratch + nin_pad;      // the product in the layout's row order, nout entries
+            // Nothing here has to start at zero: k_gather writes all nin entries of dperm before k_spmv reads them, k_spmv
+            // writes all nout entries of dres (rows without entries store 0.0) before k_scatter reads them, and neither
+            // kernel reads past nin / nout.  What an earlier call left in the array is never looked at.
+            k_gather<<<std::max(1, cdiv(nin, 256)), 256, 0, st>>>(v_device, pin, nin, dperm);
+            k_spmv<<<S.grid, kBlock, 0, st>>>(S, dperm, dres);
+            k_scatter<<<std::max(1, cdiv(nout, 256)), 256, 0, st>>>(dres, pout, nout, out_device);
+            e = cudaGetLastError();
+            if (e != cudaSuccess) rc = fail(UC_ERR_CUDA, std::string("uc_lp_spmv_static launch: ") + cudaGetErrorString(e));
+        }
+    }
+    lp->busy.store(0);
+    return rc;
+}
