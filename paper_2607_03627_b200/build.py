@@ -1,6 +1,7 @@
 """Build step: nvcc -> paper_2607_03627_b200/libuc_pdhg.so (sm_100a only, in-tree so it ships with gpurun)."""
 from __future__ import annotations
 
+import glob
 import os
 import subprocess
 
@@ -10,8 +11,10 @@ CSRC = os.path.join(HERE, "csrc")
 # the GPU tests); it is never built or rebuilt from here
 LIB = os.environ.get("UC_PDHG_LIB") or os.path.join(HERE, "libuc_pdhg.so")
 SOURCES = [os.path.join(CSRC, "uc_pdhg.cu")]
-DEPENDS = SOURCES + [os.path.join(CSRC, "uc_kernels.cuh"), os.path.join(CSRC, "uc_attempt.cuh"), os.path.join(CSRC, "uc_dd.cuh"), os.path.join(CSRC, "uc_format.hpp"),
-                     os.path.join(os.path.dirname(HERE), "include", "uc_pdhg.h")]
+# everything the translation unit includes: every file under csrc/ plus the public header (a new .cuh is picked up
+# without editing this list -- a stale library would let the GPU tests pass against old kernels)
+DEPENDS = sorted(glob.glob(os.path.join(CSRC, "*.cu")) + glob.glob(os.path.join(CSRC, "*.cuh")) + glob.glob(os.path.join(CSRC, "*.hpp"))
+                 + glob.glob(os.path.join(os.path.dirname(HERE), "include", "*.h")))
 NVCC_FLAGS = ["-O3", "-std=c++17", "-fmad=false", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared"]
 
