@@ -42,7 +42,8 @@ enum uc_error {
     UC_ERR_INVALID = -1, /* bad argument (NULL, negative size, column out of range, duplicate entry, l > u, NaN) */
     UC_ERR_CUDA = -2,    /* a CUDA runtime call or kernel failed (includes: no device) */
     UC_ERR_NOMEM = -3,   /* host or device allocation failed */
-    UC_ERR_BUSY = -4     /* a solve is already running on this handle */
+    UC_ERR_BUSY = -4,    /* a solve is already running on this handle */
+    UC_ERR_INTERNAL = -5 /* a failure inside the library that is none of the above (e.g. a helper thread could not be started) */
 };
 
 enum uc_status {
@@ -103,6 +104,13 @@ int uc_lp_update_bounds(uc_lp* lp, const double* l_new, const double* u_new);
 int uc_lp_update_objective(uc_lp* lp, const double* c_new);
 
 void uc_lp_destroy(uc_lp* lp); /* NULL ok; must not race with a solve on the same handle */
+
+/* Give back the scratch block that uc_lp_create keeps cached per device (see uc_lp_create: up to 2 GiB, ~1 GB after one
+   config-3 create; no handle owns it, so uc_lp_destroy does not free it).  device: an ordinal, or -1 = every device.
+   A block that a running uc_lp_create is using is left alone.  bytes_released (nullable) receives the bytes freed.
+   For processes that share a GPU or create once and then solve for a long time; the next uc_lp_create simply allocates
+   again.  uc_lp_info.scratch_cached_bytes reports what is held. */
+int uc_release_scratch(int32_t device, int64_t* bytes_released);
 
 /* ------------------------------------------------------------------------------------------- solve */
 /* per-attempt trace record (R5): step size used, the bound eta_bar, the next step size, the three
@@ -178,12 +186,20 @@ int uc_pdhg_solve_batch(uc_lp* const* handles, int32_t count, const uc_pdhg_para
 /* Cancel, any thread, idempotent (Algorithm 1: "Terminate the other solver").
    - A solve is in flight on the handle: THAT solve returns UC_CANCELLED at its next check (within one check
      period).  The request is scoped to it: if the solve was already past its last check and returns with
-     another status, the request is dropped -- it never leaks into a later solve on the handle.
+     another status, the request is dropped -- it never leaks into a later solve on the handle.  (A request that arrives
+     after the library has left the solve takes the second route, whatever the caller believed: uc_pdhg_cancel_clear.)
    - The handle is idle: the request is kept for the NEXT solve, which returns UC_CANCELLED at entry with
      iterations = 0 and x_out / y_out untouched -- so a cancel that lands just before the solve starts is not
      lost (the race of Algorithm 1).
    A cancel that races with the very start of a solve takes one of these two routes; both stop that solve. */
 int uc_pdhg_cancel(uc_lp* lp);
+
+/* Drop a cancel request that is being kept for the NEXT solve (second route above); a solve in flight is not affected.
+   was_pending (nullable) receives 1 if there was one.  For callers that cancel from another thread and then reuse the
+   handle: a cancel sent while the solve was returning on its own -- the caller saw its thread still alive, the library
+   had already left the solve -- would otherwise stop the next, unrelated solve at entry.  Call it after the solve has
+   returned with a status other than UC_CANCELLED (race.py does, after joining its solve thread). */
+int uc_pdhg_cancel_clear(uc_lp* lp, int32_t* was_pending);
 
 /* Measurement hook: from the initial point, run `attempts` attempts as plain stream
    launches with a CUDA event between the two kernels and return the average device time, in ms, of
@@ -214,6 +230,8 @@ typedef struct {
     double norm_b, norm_c;               /* unscaled 2-norms used by R9 */
     int64_t bytes_per_attempt;           /* bytes one attempt streams in this layout */
     int64_t k_narrow_slots, kt_narrow_slots; /* stored slots whose column index is a 16-bit offset (index_compression) */
+    int64_t scratch_cached_bytes;        /* device memory the PROCESS keeps cached on this handle's device for the next
+                                            uc_lp_create (not owned by the handle; see uc_release_scratch) */
 } uc_lp_info;
 
 int uc_lp_get_info(const uc_lp* lp, uc_lp_info* info);

@@ -5,10 +5,10 @@ the method runs in the CUDA kernels of csrc/.  There is no CPU path: without the
 or without a GPU every compute call raises.
 """
 from .binding import (UcLp, Options, Params, Result, Info, Solution, UcError, default_params, default_options,
-                      load_library, library_path, solve_batch, STATUS_NAMES,
+                      load_library, library_path, solve_batch, release_scratch, STATUS_NAMES,
                       OPTIMAL, ITERATION_LIMIT, CANCELLED, TIME_LIMIT, NUMERICAL_ERROR,
                       ATTEMPT_DTYPE, CHECK_DTYPE)
 
 __all__ = ["UcLp", "Options", "Params", "Result", "Info", "Solution", "UcError", "default_params", "default_options",
-           "load_library", "library_path", "solve_batch", "STATUS_NAMES", "OPTIMAL", "ITERATION_LIMIT", "CANCELLED", "TIME_LIMIT",
+           "load_library", "library_path", "solve_batch", "release_scratch", "STATUS_NAMES", "OPTIMAL", "ITERATION_LIMIT", "CANCELLED", "TIME_LIMIT",
            "NUMERICAL_ERROR", "ATTEMPT_DTYPE", "CHECK_DTYPE"]

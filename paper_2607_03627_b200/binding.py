@@ -51,7 +51,8 @@ class Info(C.Structure):
                 ("k_long_nnz", C.c_int64), ("kt_long_nnz", C.c_int64), ("device_bytes", C.c_int64),
                 ("precondition_seconds", C.c_double), ("create_seconds", C.c_double),
                 ("eta0", C.c_double), ("omega0", C.c_double), ("norm_b", C.c_double), ("norm_c", C.c_double),
-                ("bytes_per_attempt", C.c_int64), ("k_narrow_slots", C.c_int64), ("kt_narrow_slots", C.c_int64)]
+                ("bytes_per_attempt", C.c_int64), ("k_narrow_slots", C.c_int64), ("kt_narrow_slots", C.c_int64),
+                ("scratch_cached_bytes", C.c_int64)]
 
 
 ATTEMPT_DTYPE = np.dtype([("eta_used", "f8"), ("eta_bar", "f8"), ("eta_next", "f8"), ("dx2", "f8"),
@@ -61,8 +62,8 @@ CHECK_DTYPE = np.dtype([("k", "i8"), ("restart_kind", "i4"), ("candidate", "i4")
 
 SPMV_STATIC_MAX_DOUBLES = 262144      # UC_SPMV_STATIC_MAX_DOUBLES of include/uc_pdhg.h
 
-EXPORTS = ["uc_lp_default_options", "uc_lp_create", "uc_lp_update_bounds", "uc_lp_update_objective", "uc_lp_destroy",
-           "uc_pdhg_default_params", "uc_pdhg_solve", "uc_pdhg_solve_device", "uc_pdhg_solve_batch", "uc_pdhg_cancel", "uc_pdhg_time_kernels", "uc_pdhg_timeline", "uc_lp_compare_layout",
+EXPORTS = ["uc_lp_default_options", "uc_lp_create", "uc_lp_update_bounds", "uc_lp_update_objective", "uc_lp_destroy", "uc_release_scratch",
+           "uc_pdhg_default_params", "uc_pdhg_solve", "uc_pdhg_solve_device", "uc_pdhg_solve_batch", "uc_pdhg_cancel", "uc_pdhg_cancel_clear", "uc_pdhg_time_kernels", "uc_pdhg_timeline", "uc_lp_compare_layout",
            "uc_lp_get_info", "uc_lp_get_scaling", "uc_lp_get_scaled_values", "uc_lp_spmv", "uc_lp_spmv_static", "uc_last_error",
            "uc_host_log_rounded", "uc_host_exp_rounded", "uc_host_layout_selftest"]
 
@@ -107,6 +108,8 @@ def load_library(build_if_missing: bool = True):
     lib.uc_lp_get_scaling.argtypes = [C.c_void_p] * 3
     lib.uc_lp_get_scaled_values.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
     lib.uc_lp_spmv.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
+    lib.uc_pdhg_cancel_clear.argtypes = [C.c_void_p, C.c_void_p]
+    lib.uc_release_scratch.argtypes = [C.c_int32, C.c_void_p]
     lib.uc_lp_spmv_static.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
     _lib = lib
     return lib
@@ -124,6 +127,13 @@ def host_layout_selftest(lp, sell_window=4096, long_row_threshold=32, sched_ctas
     va = np.ascontiguousarray(lp.val, dtype=np.float64)
     _check(lib.uc_host_layout_selftest(int(lp.m), int(lp.n), int(lp.nnz), C.c_void_p(rp.ctypes.data), C.c_void_p(ci.ctypes.data),
                                        C.c_void_p(va.ctypes.data), int(sell_window), int(long_row_threshold), int(sched_ctas), int(warps_per_cta)))
+
+
+def release_scratch(device: int = -1) -> int:
+    """uc_release_scratch: free the per-device scratch block that uc_lp_create keeps cached; returns the bytes freed."""
+    n = C.c_int64(0)
+    _check(load_library().uc_release_scratch(int(device), C.cast(C.byref(n), C.c_void_p)))
+    return int(n.value)
 
 
 def default_options(**kw) -> Options:
@@ -228,6 +238,14 @@ class UcLp:
         _check(self.lib.uc_pdhg_cancel(self._h))
 
     cancel = uc_pdhg_cancel
+
+    def uc_pdhg_cancel_clear(self) -> bool:
+        """Drop a cancel request kept for the next solve; True if there was one."""
+        had = C.c_int32(0)
+        _check(self.lib.uc_pdhg_cancel_clear(self._h, C.cast(C.byref(had), C.c_void_p)))
+        return bool(had.value)
+
+    cancel_clear = uc_pdhg_cancel_clear
 
     def uc_lp_update_bounds(self, l, u):
         la, lp_ = _host(l, np.float64)

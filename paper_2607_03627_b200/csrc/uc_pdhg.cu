@@ -35,6 +35,12 @@ struct TooLarge { const char* what; };                            // a size limi
         if (e__ != cudaSuccess) throw CudaFail{e__, #call};      \
     } while (0)
 
+// code of a standard exception caught at the ABI: allocation failures keep UC_ERR_NOMEM, everything else (std::system_error
+// of a helper thread, std::length_error, ...) is an internal failure with its own code
+int std_code(const std::exception& e) {
+    return (dynamic_cast<const std::bad_alloc*>(&e) || dynamic_cast<const std::bad_array_new_length*>(&e)) ? UC_ERR_NOMEM : UC_ERR_INTERNAL;
+}
+
 double now_s() {
     return std::chrono::duration<double>(std::chrono::steady_clock::now().time_since_epoch()).count();
 }
@@ -59,6 +65,11 @@ struct uc_lp {
     // warm start after it came from them.  Owned by the handle: no cudaMalloc / cudaFree on the solve path (they
     // synchronise the device and were seen to stall for hundreds of ms now and then).
     double *stage_x = nullptr, *stage_y = nullptr, *stage_x0 = nullptr, *stage_y0 = nullptr;
+    // scratch of uc_lp_update_bounds / uc_lp_update_objective, allocated by the first such call and kept: re-solve loops
+    // call them once per node, and a cudaMalloc / cudaFree pair per call stalls the device (see above).  The n-vectors of
+    // those calls are stage_x (always there) and stage_x0 (allocated on first need); nothing else uses them while the
+    // handle's busy flag is held.
+    dd* upd_part = nullptr; double* upd_scal = nullptr;
     double *qs = nullptr, *cs = nullptr, *ls = nullptr, *us = nullptr;
     unsigned char* isG = nullptr;
     // host <-> device mailboxes (pinned, mapped)
@@ -179,8 +190,14 @@ struct TempArena {
     struct Cache { std::mutex mu; std::vector<void*> base; std::vector<size_t> cap; std::vector<char> busy; };
     static Cache& cache() { static Cache c; return c; }
     char* base = nullptr; size_t cap = 0, used = 0; int dev = -1; bool cached = false;
+    // set by uc_lp_create after its last stream synchronisation: nothing enqueued can still touch the block.  On every
+    // other way out (an exception, a validation failure after the copies were enqueued) copies and ingest kernels may
+    // still be running, on the handle's stream or the upload thread's, and the handle's stream may already be destroyed:
+    // the destructor then waits for the whole device before the block can be handed to the next uc_lp_create or freed.
+    bool quiesced = false;
     ~TempArena() {
         if (!base) return;
+        if (!quiesced) cudaDeviceSynchronize();          // the creating thread still has the arena's device current
         Cache& C = cache();
         std::lock_guard<std::mutex> g(C.mu);
         if (cached) { C.busy[(size_t)dev] = 0; return; }                     // back to the cache
@@ -188,6 +205,27 @@ struct TempArena {
             if (C.base[(size_t)dev]) cudaFree(C.base[(size_t)dev]);
             C.base[(size_t)dev] = base; C.cap[(size_t)dev] = cap;
         } else cudaFree(base);
+    }
+    // bytes the cache holds for `device` right now (in use by a running uc_lp_create or not)
+    static size_t cached_bytes(int device) {
+        Cache& C = cache();
+        std::lock_guard<std::mutex> g(C.mu);
+        return device >= 0 && device < (int)C.base.size() && C.base[(size_t)device] ? C.cap[(size_t)device] : 0;
+    }
+    // free the cached block of `device` (-1: of every device) unless a uc_lp_create is using it; returns the bytes freed
+    static size_t release(int device) {
+        Cache& C = cache();
+        std::lock_guard<std::mutex> g(C.mu);
+        size_t freed = 0;
+        int prev = -1; cudaGetDevice(&prev);
+        for (int d = 0; d < (int)C.base.size(); ++d) {
+            if ((device >= 0 && d != device) || !C.base[(size_t)d] || C.busy[(size_t)d]) continue;
+            cudaSetDevice(d);
+            cudaFree(C.base[(size_t)d]);
+            freed += C.cap[(size_t)d]; C.base[(size_t)d] = nullptr; C.cap[(size_t)d] = 0;
+        }
+        if (prev >= 0) cudaSetDevice(prev);
+        return freed;
     }
     void reserve(size_t bytes, int device) {
         dev = device;
@@ -672,7 +710,7 @@ int uc_host_layout_selftest(int64_t m, int64_t n, int64_t nnz, const int64_t* ro
     w = check_sell(P.KT, true);
     if (!w.empty()) return bad("K' layout: " + w);
     } catch (const std::exception& e) {                        // nothing may unwind through the C ABI
-        return fail(UC_ERR_NOMEM, std::string("uc_host_layout_selftest: ") + e.what());
+        return fail(std_code(e), std::string("uc_host_layout_selftest: ") + e.what());
     }
     return UC_OK;
 }
@@ -943,6 +981,7 @@ int uc_lp_create(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, cons
         double hs[6];
         CK(cudaMemcpyAsync(hs, scal, sizeof hs, cudaMemcpyDeviceToHost, st));
         CK(cudaStreamSynchronize(st));
+        T.quiesced = true;                               // last use of the temporary arena (scal, part) is done
         float ms = 0.f; CK(cudaEventElapsedTime(&ms, lp->ev_t0, lp->ev_t1));
         lp->precondition_seconds = ms * 1e-3;
         lp->norm_b = std::sqrt(hs[0]); lp->norm_c = std::sqrt(hs[1]);
@@ -969,7 +1008,7 @@ int uc_lp_create(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, cons
     } catch (const std::exception& e) {                       // std::system_error of a helper thread, std::length_error, ...
         join_validation();
         destroy_impl(lp);
-        return fail(UC_ERR_NOMEM, std::string("uc_lp_create: ") + e.what());
+        return fail(std_code(e), std::string("uc_lp_create: ") + e.what());
     }
     join_validation();
     *out = lp;
@@ -977,6 +1016,13 @@ int uc_lp_create(int64_t m, int64_t n, int64_t nnz, const int64_t* row_ptr, cons
 }
 
 void uc_lp_destroy(uc_lp* lp) { destroy_impl(lp); }
+
+int uc_release_scratch(int32_t device, int64_t* bytes_released) {
+    if (device < -1) return fail(UC_ERR_INVALID, "uc_release_scratch: device must be an ordinal or -1");
+    const size_t freed = TempArena::release(device);
+    if (bytes_released) *bytes_released = (int64_t)freed;
+    return UC_OK;
+}
 
 int uc_lp_update_bounds(uc_lp* lp, const double* l_new, const double* u_new) {
     if (!lp || (lp->n > 0 && (!l_new || !u_new))) return fail(UC_ERR_INVALID, "NULL argument");
@@ -987,14 +1033,17 @@ int uc_lp_update_bounds(uc_lp* lp, const double* l_new, const double* u_new) {
     int rc = UC_OK;
     try {
         DeviceGuard guard(lp->device);
-        double *dl = nullptr, *du = nullptr;
-        size_t bytes = sizeof(double) * (size_t)std::max<int64_t>(lp->n, 1);
-        CK(cudaMalloc((void**)&dl, bytes)); CK(cudaMalloc((void**)&du, bytes));
-        if (lp->n) { CK(cudaMemcpy(dl, l_new, sizeof(double) * (size_t)lp->n, cudaMemcpyHostToDevice)); CK(cudaMemcpy(du, u_new, sizeof(double) * (size_t)lp->n, cudaMemcpyHostToDevice)); }
+        if (!lp->stage_x0) lp->stage_x0 = lp->dalloc<double>((size_t)lp->n);          // first use on this handle; kept
+        double *dl = lp->stage_x, *du = lp->stage_x0;
+        // on the handle's stream (a non-blocking one: a copy on the legacy stream would not be ordered before the kernel,
+        // nor after the zero-fill of a fresh stage_x0)
+        if (lp->n) {
+            CK(cudaMemcpyAsync(dl, l_new, sizeof(double) * (size_t)lp->n, cudaMemcpyHostToDevice, lp->own_stream));
+            CK(cudaMemcpyAsync(du, u_new, sizeof(double) * (size_t)lp->n, cudaMemcpyHostToDevice, lp->own_stream));
+        }
         k_scale_bounds<<<std::max(1, cdiv(lp->n, kBlock)), kBlock, 0, lp->own_stream>>>(lp->n, dl, du, lp->perm_c, lp->Dc, lp->ls, lp->us);
         CK(cudaGetLastError());
         CK(cudaStreamSynchronize(lp->own_stream));
-        cudaFree(dl); cudaFree(du);
     } catch (const CudaFail& f) {
         rc = fail(UC_ERR_CUDA, std::string(f.what) + ": " + cudaGetErrorString(f.e));
     }
@@ -1009,12 +1058,11 @@ int uc_lp_update_objective(uc_lp* lp, const double* c_new) {
     int expected = 0;
     if (!lp->busy.compare_exchange_strong(expected, 1)) return fail(UC_ERR_BUSY, "a solve is running on this handle");
     int rc = UC_OK;
-    double* dc = nullptr; dd* part = nullptr; double* scal = nullptr;
     try {
         DeviceGuard guard(lp->device);
         cudaStream_t st = lp->own_stream;
-        const size_t bytes = sizeof(double) * (size_t)std::max<int64_t>(lp->n, 1);
-        CK(cudaMalloc((void**)&dc, bytes)); CK(cudaMalloc((void**)&part, sizeof(dd) * 1024)); CK(cudaMalloc((void**)&scal, sizeof(double)));
+        if (!lp->upd_part) { lp->upd_part = lp->dalloc<dd>(1024); lp->upd_scal = lp->dalloc<double>(8); }   // first call on this handle; kept
+        double* dc = lp->stage_x; dd* part = lp->upd_part; double* scal = lp->upd_scal;
         if (lp->n) CK(cudaMemcpyAsync(dc, c_new, sizeof(double) * (size_t)lp->n, cudaMemcpyHostToDevice, st));
         lp->norm_c = std::sqrt(reduce_to_host(lp, dc, lp->n, 0, part, scal, st));            // unscaled ||c|| of R9
         k_scale_cost<<<std::max(1, cdiv(lp->n, kBlock)), kBlock, 0, st>>>(lp->n, dc, lp->perm_c, lp->Dc, lp->cs);
@@ -1024,9 +1072,6 @@ int uc_lp_update_objective(uc_lp* lp, const double* c_new) {
     } catch (const CudaFail& f) {
         rc = fail(UC_ERR_CUDA, std::string(f.what) + ": " + cudaGetErrorString(f.e));
     }
-    if (dc) cudaFree(dc);
-    if (part) cudaFree(part);
-    if (scal) cudaFree(scal);
     lp->busy.store(0);
     return rc;
 }
@@ -1036,6 +1081,13 @@ int uc_pdhg_cancel(uc_lp* lp) {
     const unsigned st = lp->state.load();
     if ((st & 1u) && lp->h_stop) __atomic_store_n(lp->h_stop, (int)(((st >> 1) & 0x0fffffffu) << 3) | UC_CANCELLED, __ATOMIC_SEQ_CST);
     else lp->cancel_requested.store(1);
+    return UC_OK;
+}
+
+int uc_pdhg_cancel_clear(uc_lp* lp, int32_t* was_pending) {
+    if (!lp) return fail(UC_ERR_INVALID, "handle is NULL");
+    const int had = lp->cancel_requested.exchange(0);
+    if (was_pending) *was_pending = had;
     return UC_OK;
 }
 
@@ -1170,7 +1222,7 @@ static int solve_impl(uc_lp* lp, const uc_pdhg_params* pin, double* x_out, doubl
     } catch (const CudaFail& f) {
         rc = fail((f.e == cudaErrorMemoryAllocation) ? UC_ERR_NOMEM : UC_ERR_CUDA, std::string(f.what) + ": " + cudaGetErrorString(f.e));
     } catch (const std::exception& e) {                        // nothing may unwind through the C ABI
-        rc = fail(UC_ERR_NOMEM, std::string("uc_pdhg_solve: ") + e.what());
+        rc = fail(std_code(e), std::string("uc_pdhg_solve: ") + e.what());
     }
     if (d_att) cudaFree(d_att);
     if (d_chk) cudaFree(d_chk);
@@ -1213,14 +1265,20 @@ int uc_pdhg_solve_batch(uc_lp* const* handles, int32_t count, const uc_pdhg_para
             if (rcs[(size_t)i] != UC_OK) errs[(size_t)i] = g_err;       // thread-local text of the worker
         }
     };
-    try {
-        std::vector<std::thread> th;
-        for (int w = 1; w < workers; ++w) th.emplace_back(work);
-        work();
-        for (auto& t : th) t.join();
-    } catch (const std::exception& e) {
-        return fail(UC_ERR_NOMEM, std::string("uc_pdhg_solve_batch: ") + e.what());
+    // Workers are joined on every way out of this scope: a std::thread that is destroyed while joinable ends the process,
+    // and nothing may unwind through the C ABI.  If a worker cannot be started (std::system_error), the ones that did start
+    // and the calling thread drain the queue between them.
+    struct Pool { std::vector<std::thread> th; ~Pool() { for (auto& t : th) if (t.joinable()) t.join(); } };
+    std::string spawn_err; int spawn_code = UC_ERR_INTERNAL;
+    {
+        Pool pool;
+        try {
+            pool.th.reserve((size_t)workers);
+            for (int w = 1; w < workers; ++w) pool.th.emplace_back(work);
+        } catch (const std::exception&) { /* fewer workers than asked for */ }
+        try { work(); } catch (const std::exception& e) { spawn_err = e.what(); spawn_code = std_code(e); next.store(count); }
     }
+    if (!spawn_err.empty()) return fail(spawn_code, "uc_pdhg_solve_batch: " + spawn_err);
     for (int32_t i = 0; i < count; ++i)
         if (rcs[(size_t)i] != UC_OK) return fail(rcs[(size_t)i], "solve " + std::to_string(i) + ": " + errs[(size_t)i]);
     return UC_OK;
@@ -1318,6 +1376,7 @@ int uc_lp_get_info(const uc_lp* lp, uc_lp_info* info) {
     info->eta0 = lp->eta0; info->omega0 = lp->omega0; info->norm_b = lp->norm_b; info->norm_c = lp->norm_c;
     info->bytes_per_attempt = bytes_per_attempt(lp);
     info->k_narrow_slots = lp->k_narrow; info->kt_narrow_slots = lp->kt_narrow;
+    info->scratch_cached_bytes = (int64_t)TempArena::cached_bytes(lp->device);
     return UC_OK;
 }
 
@@ -1378,7 +1437,7 @@ int uc_lp_compare_layout(uc_lp* lp, int64_t m, int64_t n, int64_t nnz, const int
     } catch (const CudaFail& f) {
         return fail(UC_ERR_CUDA, std::string(f.what) + ": " + cudaGetErrorString(f.e));
     } catch (const std::exception& e) {
-        return fail(UC_ERR_NOMEM, e.what());
+        return fail(std_code(e), e.what());
     }
     return UC_OK;
 }
@@ -1405,7 +1464,7 @@ int uc_lp_get_scaling(uc_lp* lp, double* Dr_out, double* Dc_out) {
     } catch (const CudaFail& f) {
         return fail(UC_ERR_CUDA, std::string(f.what) + ": " + cudaGetErrorString(f.e));
     } catch (const std::exception& e) {                        // nothing may unwind through the C ABI
-        return fail(UC_ERR_NOMEM, e.what());
+        return fail(std_code(e), e.what());
     }
     return UC_OK;
 }
@@ -1427,7 +1486,7 @@ int uc_lp_get_scaled_values(uc_lp* lp, int32_t from_transpose, double* val_out) 
     } catch (const CudaFail& f) {
         return fail(UC_ERR_CUDA, std::string(f.what) + ": " + cudaGetErrorString(f.e));
     } catch (const std::exception& e) {                        // nothing may unwind through the C ABI
-        return fail(UC_ERR_NOMEM, e.what());
+        return fail(std_code(e), e.what());
     }
     return UC_OK;
 }

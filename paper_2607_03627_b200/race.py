@@ -148,6 +148,12 @@ def race(handle: "_b.UcLp", competitor: Callable[..., Any], competitor_args: tup
             th.join()
             res.cancel_latency_s = time.perf_counter() - tc
             res.log.append("uc_pdhg_cancel sent")
+            # The thread being alive does not mean the library is still inside the solve: a cancel that lands after the
+            # solve has left its loop is kept for the NEXT solve on the handle (uc_pdhg.h), and callers reuse handles
+            # (re-solves, the "GPU alone" column of _main).  The solve returned on its own, so drop that request.
+            sol = box.get("sol")
+            if (sol is None or sol.status != _b.CANCELLED) and hasattr(handle, "cancel_clear") and handle.cancel_clear():
+                res.log.append("cancel arrived after the GPU solve had returned: request dropped")
     else:
         th.join()
         if proc.is_alive():

@@ -41,6 +41,56 @@ def test_default_structs_match_header_values():
     assert p.check_every == 64 and p.fixed_iterations == 0 and not p.x0 and not p.stream
 
 
+def test_struct_layouts_match_a_c_client_compiled_against_the_header(tmp_path):
+    """A C11 client built with gcc against include/uc_pdhg.h prints sizeof and every offsetof; the ctypes Structures and the
+    numpy record dtypes of the binding must give the same numbers (a reordered field of equal type would pass a
+    default-value check, not this one)."""
+    import shutil
+    import subprocess
+    structs = {"uc_lp_options": binding.Options, "uc_pdhg_params": binding.Params, "uc_pdhg_result": binding.Result,
+               "uc_lp_info": binding.Info}
+    records = {"uc_attempt_record": binding.ATTEMPT_DTYPE, "uc_check_record": binding.CHECK_DTYPE}
+    lines = ["#include <stdio.h>", "#include <stddef.h>", '#include "uc_pdhg.h"', "int main(void) {"]
+    for name, st in structs.items():
+        lines.append(f'printf("{name} size %zu\\n", sizeof({name}));')
+        lines += [f'printf("{name} {f} %zu\\n", offsetof({name}, {f}));' for f, _ in st._fields_]
+    for name, dt in records.items():
+        lines.append(f'printf("{name} size %zu\\n", sizeof({name}));')
+        lines += [f'printf("{name} {f} %zu\\n", offsetof({name}, {f}));' for f in dt.names]
+    lines += ['printf("UC_SPMV_STATIC_MAX_DOUBLES size %d\\n", (int)UC_SPMV_STATIC_MAX_DOUBLES);', "return 0; }"]
+    src = tmp_path / "client.c"; exe = tmp_path / "client"
+    src.write_text("\n".join(lines))
+    gcc = shutil.which("gcc")
+    assert gcc, "gcc is part of the image"
+    subprocess.check_call([gcc, "-std=c11", "-Wall", "-Werror", "-I", os.path.join(ROOT, "include"), "-o", str(exe), str(src)])
+    got = {}
+    for ln in subprocess.check_output([str(exe)], text=True).splitlines():
+        a, b, c = ln.split()
+        got[(a, b)] = int(c)
+    for name, st in structs.items():
+        assert got[(name, "size")] == C.sizeof(st), name
+        for f, _ in st._fields_:
+            assert got[(name, f)] == getattr(st, f).offset, (name, f)
+    for name, dt in records.items():
+        assert got[(name, "size")] == dt.itemsize, name
+        for f in dt.names:
+            assert got[(name, f)] == dt.fields[f][1], (name, f)
+    assert got[("UC_SPMV_STATIC_MAX_DOUBLES", "size")] == binding.SPMV_STATIC_MAX_DOUBLES
+    # and the header declares exactly the fields the binding knows (a field added on one side only fails here)
+    hdr = re.sub(r"/\*.*?\*/", "", open(os.path.join(ROOT, "include", "uc_pdhg.h")).read(), flags=re.S)
+    for name, st in list(structs.items()) + [(k, None) for k in records]:
+        body = re.search(r"typedef struct \{([^}]*)\} " + name + ";", hdr).group(1)
+        declared = []
+        for decl in body.split(";"):
+            decl = decl.strip()
+            if not decl:
+                continue
+            names = decl.split(None, 1)[1] if not decl.startswith("const") else decl.split(None, 2)[2]
+            declared += [t.strip().lstrip("*").strip() for t in names.split(",")]
+        want = [f for f, _ in st._fields_] if st is not None else list(records[name].names)
+        assert declared == want, name
+
+
 def _create_raw(lp, **over):
     lib = P.load_library()
     a = dict(row_ptr=lp.row_ptr, col_idx=lp.col_idx, val=lp.val, sense=lp.sense, b=lp.b, c=lp.c, l=lp.l, u=lp.u)

@@ -56,6 +56,46 @@ def test_cancel_from_another_thread_stops_within_a_few_checks(lp1):
         assert again.status == P.ITERATION_LIMIT
 
 
+def test_cancel_clear_drops_a_request_sent_after_the_solve_returned(lp1):
+    with P.UcLp(lp1) as h:
+        assert h.solve(fixed_iterations=64).status == P.ITERATION_LIMIT
+        assert h.cancel_clear() is False                   # nothing pending
+        h.cancel()                                         # too late for that solve: kept for the next one ...
+        assert h.cancel_clear() is True                    # ... unless the caller says it was meant for the last one
+        s = h.solve(fixed_iterations=64)
+        assert s.status == P.ITERATION_LIMIT and s.iterations == 64
+
+
+def test_release_scratch_frees_the_cached_create_block_and_create_still_works(lp1):
+    with P.UcLp(lp1) as h:
+        held = h.info().scratch_cached_bytes
+        assert held > 0                                    # uc_lp_create keeps its scratch block for the next create
+        ref = h.solve(fixed_iterations=64)
+        assert P.release_scratch(-1) == held
+        assert h.info().scratch_cached_bytes == 0 and P.release_scratch(-1) == 0
+        with P.UcLp(lp1) as h2:                            # allocates again, same result
+            again = h2.solve(fixed_iterations=64)
+            assert h2.info().scratch_cached_bytes > 0
+        assert np.array_equal(ref.x, again.x) and np.array_equal(ref.y, again.y)
+
+
+def test_create_rejected_after_its_copies_were_enqueued_leaves_the_scratch_cache_usable(lp1):
+    """A duplicate entry is found by the validation thread while the H2D copies of the CSR are already enqueued on the
+    handle's stream; the scratch block must not go back to the cache (and to the next create) before they are done."""
+    bad_cols = lp1.col_idx.copy()
+    r0 = int(np.argmax(np.diff(lp1.row_ptr) >= 2)); p0 = int(lp1.row_ptr[r0])
+    bad_cols[p0 + 1] = bad_cols[p0]                        # duplicate (row, col)
+    import copy
+    bad = copy.copy(lp1); bad.col_idx = bad_cols
+    for _ in range(3):
+        with pytest.raises(P.UcError) as e:
+            P.UcLp(bad)
+        assert e.value.code == -1
+        with P.UcLp(lp1) as h:
+            h.uc_lp_compare_layout(lp1)                       # what the device holds is the good LP's layout, bit for bit
+            assert h.solve(fixed_iterations=64).iterations == 64
+
+
 def test_time_limit(lp1):
     with P.UcLp(lp1) as h:
         s = h.solve(iter_limit=50_000_000, eps_rel=0.0, eps_abs=0.0, time_limit_s=0.3)

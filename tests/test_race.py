@@ -29,6 +29,31 @@ class StandInHandle:
         self._stop.set()
 
 
+class LateCancelHandle(StandInHandle):
+    """The window of the real library: solve() has left its loop (status decided, not CANCELLED) while its thread is still
+    alive, so a cancel() sent now is parked for the next solve -- unless cancel_clear() drops it."""
+
+    def __init__(self):
+        super().__init__(seconds=0.0, final_status=B.ITERATION_LIMIT)
+        self.left_loop, self.parked, self.cleared = threading.Event(), False, False
+
+    def solve(self, **kw):
+        if self.parked:                                        # what uc_pdhg_solve does with a parked request
+            self.parked = False
+            return SimpleNamespace(status=B.CANCELLED, primal_obj=0.0, iterations=0)
+        self.left_loop.set()
+        self._stop.wait(30.0)                                  # thread alive until the cancel arrives
+        return SimpleNamespace(status=B.ITERATION_LIMIT, primal_obj=self.objective, iterations=64)
+
+    def cancel(self):
+        self.cancelled = self.parked = True
+        self._stop.set()
+
+    def cancel_clear(self):
+        had, self.parked, self.cleared = self.parked, False, True
+        return had
+
+
 def slow_competitor(seconds, value):
     time.sleep(seconds)
     return value
@@ -47,6 +72,14 @@ def test_cpu_wins_and_the_gpu_side_is_cancelled_through_its_hook():
     assert h.cancelled and r.gpu.status == B.CANCELLED
     assert r.cancel_latency_s is not None and r.cancel_latency_s < 1.0
     assert r.seconds < 5.0 and r.cpu_seconds is not None
+
+
+def test_a_cancel_that_misses_the_solve_does_not_leak_into_the_next_one():
+    h = LateCancelHandle()
+    r = race(h, slow_competitor, (0.2, 7.5), poll_s=0.05)
+    assert r.winner == "cpu" and h.cancelled and r.gpu.status == B.ITERATION_LIMIT
+    assert h.cleared and not h.parked and any("request dropped" in m for m in r.log)
+    assert h.solve().status == B.ITERATION_LIMIT               # the handle is reusable: no CANCELLED at entry
 
 
 def test_gpu_wins_and_the_competitor_process_is_terminated():
