@@ -330,11 +330,20 @@ def main():
         att_ms = 1e3 * loop_s / (args.steps * A)
         traffic, traffic_src = ncu_traffic(args.config)
         tr = traffic.get(dom[0]) if traffic else None
+        ncu_us = traffic.get(dom[0] + "_us_ncu") if traffic else None
         roof = {"bound": "hbm", "kernel": dom[0], "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                "what": "effective bandwidth: ALGORITHMIC bytes of the kernel / its CUDA-event time; frac_dram is the same with the "
-                        "DRAM bytes ncu measured (gathers served from L2 are not DRAM traffic)",
+                "what": "frac = effective_frac: ALGORITHMIC bytes of the kernel / its CUDA-event time / the measured copy bandwidth. "
+                        "It is NOT the DRAM utilisation: part of the algorithmic bytes (the gathers, the evict_last vectors) is served "
+                        "from L2; frac_dram is the same quotient with the DRAM bytes ncu measured.  The ceiling named by \"bound\" is the "
+                        "one the byte count is held against; the limiter ncu shows for both attempt kernels is the L2 request rate of "
+                        "the 8/16-byte gathers (DESIGN.md section 7), with DRAM at 42-54 % of its peak",
+                "effective_frac": ach / peak, "limiter": "l2_requests_of_the_gathers",
                 "traffic": tr, "traffic_source": traffic_src if tr else None,
                 "frac_dram": (tr / (dom[2] * 1e-3) / 1e9 / peak) if tr else None,
+                "kernel_ms_ncu": (ncu_us * 1e-3) if ncu_us else None,
+                "kernel_ms_note": "kernel_ms: CUDA events around the kernel with an event record between the two kernels (keeps the next "
+                                  "kernel from starting early, so it is an upper bound); kernel_ms_ncu: gpu__time_duration of the same kernel in "
+                                  "the committed launch list (cold cache, serialised); in_graph.pair_ms: both kernels inside the graph",
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": dom[1], "kernel_ms": dom[2],
                 "other_kernel": {"k_primal_ms": primal_ms, "k_dual_ms": dual_ms, "k_primal_bytes": bp, "k_dual_bytes": bd},
                 "in_graph": {"what": "context for kernel_ms: an event record between two kernels keeps the next one from starting early "
