@@ -439,6 +439,71 @@ def test_status_codes_and_iteration_accounting():
     assert len(s.checks) == 3 and s.returned_average == 0
 
 
+# ------------------------------------------------------------------ R12 with eps_abs != eps_rel; which point a capped run returns
+def _dense_terms(lp, s, i):
+    """dense_kkt of the current iterate and of the average that check i of an oracle run saw (unscaled from its dumps)."""
+    cur = dense_kkt(lp, s.check_x[i] / s.Dc, s.check_y[i] / s.Dr)
+    avg = dense_kkt(lp, s.check_avg_x[i] / s.Dc, s.check_avg_y[i] / s.Dr)
+    return cur, avg
+
+
+def _passes(lp, k, ea, er):
+    """R12 / SURVEY O5 written out: ||r_p|| <= ea + er ||q||, ||r_d|| <= ea + er ||c||, |gap| <= ea + er (|p| + |d|)."""
+    return (k["rp"] <= ea + er * np.linalg.norm(lp.b) and k["rd"] <= ea + er * np.linalg.norm(lp.c) and
+            abs(k["pobj"] - k["dobj"]) <= ea + er * (abs(k["pobj"]) + abs(k["dobj"])))
+
+
+@pytest.mark.parametrize("name", ["small_random", "uc0"])
+@pytest.mark.parametrize("ea,er", [(1e-3, 1e-9), (1e-9, 1e-3), (1e-5, 1e-4)])
+def test_termination_with_separate_absolute_and_relative_tolerances(name, ea, er):
+    """PAPER.md l.66 sets an ABSOLUTE feasibility tolerance (1e-5) next to the relative 1e-4 of l.91, so eps_abs and eps_rel
+    differ in the paper's own runs.  From the iterates the oracle dumped at every check, dense numpy algebra decides where
+    the run had to stop: at the FIRST check whose average or current iterate passes R12 with (ea, er) in their own places.
+    The oracle with the two swapped (or one used for both) stops at a different check on these LPs -- asserted below, so
+    the case really separates them."""
+    lp = tiny.small_random(6, 4, 1) if name == "small_random" else uc_config(0)
+    s = oracle.solve(lp, eps_abs=ea, eps_rel=er, iter_limit=400000, dump_checks=8192, trace_checks=8192)
+    assert s.status == 0 and len(s.check_x) == len(s.checks) < 8192
+    last = len(s.checks) - 1
+    for i in range(last + 1):
+        cur, avg = _dense_terms(lp, s, i)
+        ok_avg, ok_cur = _passes(lp, avg, ea, er), _passes(lp, cur, ea, er)
+        if i < last:
+            # a borderline value (within rounding of the threshold) would make this comparison of two different
+            # summation orders meaningless; none occurs on these LPs
+            assert not ok_avg and not ok_cur, f"check {i} already passes but the oracle went on"
+        else:
+            assert ok_avg or ok_cur, "oracle stopped at a check that does not pass"
+            assert s.returned_average == (1 if ok_avg else 0)           # the average is tried first (R12)
+    if ea != er and not (ea, er) == (1e-5, 1e-4):
+        swapped = oracle.solve(lp, eps_abs=er, eps_rel=ea, iter_limit=400000)
+        assert swapped.iterations != s.iterations                        # the pair is not symmetric on this LP
+
+
+@pytest.mark.parametrize("name,limit", [("uc0", 100), ("uc0", 640), ("small_random", 64), ("small_random", 192)])
+def test_a_run_that_hits_its_iteration_limit_returns_the_better_of_current_and_average(name, limit):
+    """R12 / SURVEY O5: on a non-OPTIMAL exit the point handed back is whichever of the current iterate and the average has
+    the smaller relative KKT error at the last check (ties: the current one).  Decided here by dense numpy algebra on the
+    dumped iterates, with the relative KKT error written out from its definition (R9)."""
+    lp = tiny.small_random(6, 4, 1) if name == "small_random" else uc_config(0)
+    s = oracle.solve(lp, iter_limit=limit, eps_abs=0.0, eps_rel=0.0, dump_checks=64, trace_checks=64)
+    assert s.status == 1 and s.iterations == limit and int(s.checks["k"][-1]) == limit
+    cur, avg = _dense_terms(lp, s, len(s.checks) - 1)
+
+    def rel(k):
+        return max(k["rp"] / (1 + np.linalg.norm(lp.b)), k["rd"] / (1 + np.linalg.norm(lp.c)),
+                   abs(k["pobj"] - k["dobj"]) / (1 + abs(k["pobj"]) + abs(k["dobj"])))
+    rc, ra = rel(cur), rel(avg)
+    assert abs(rc - ra) > 1e-9 * max(rc, ra)                             # not a tie: the choice is decided
+    want_avg = ra < rc and s.check_w[-1] > 0.0
+    assert s.returned_average == int(want_avg)
+    i = len(s.checks) - 1
+    xs, ys = (s.check_avg_x[i], s.check_avg_y[i]) if want_avg else (s.check_x[i], s.check_y[i])
+    np.testing.assert_array_equal(s.x, xs / s.Dc)
+    np.testing.assert_array_equal(s.y, ys / s.Dr)
+    assert s.rel_kkt == pytest.approx(min(rc, ra) if s.check_w[-1] > 0.0 else rc, rel=1e-6)
+
+
 # ------------------------------------------------------------------ library cross-check on the UC LP
 def test_uc_config0_converges_to_highs_objective():
     lp = uc_config(0)
