@@ -45,6 +45,24 @@ def ragged_lp(seed=5, n=3000, m=2500):
     return lp
 
 
+def shuffled_in_rows(lp, seed):
+    """The same LP with the entries of every row in a random order (include/uc_pdhg.h: "order inside a row is free").
+    Built here on the raw CSR arrays: workloads.lp.from_coo would sort the columns again.  The sum of a row follows the
+    caller's storage order on both sides, so the oracle is given the shuffled LP too and parity stays bit-level."""
+    import copy
+    rng = np.random.default_rng(seed)
+    q = copy.copy(lp)
+    q.col_idx = lp.col_idx.copy(); q.val = lp.val.copy()
+    for i in range(lp.m):
+        a, b = int(lp.row_ptr[i]), int(lp.row_ptr[i + 1])
+        if b - a > 1:
+            p = a + rng.permutation(b - a)
+            q.col_idx[a:b] = lp.col_idx[p]; q.val[a:b] = lp.val[p]
+    assert any(np.any(np.diff(q.col_idx[int(q.row_ptr[i]):int(q.row_ptr[i + 1])]) < 0) for i in range(min(lp.m, 200)))
+    q.name = lp.name + "_shuffled"
+    return q
+
+
 CASES = {
     "one_by_one": tiny.one_by_one,
     "two_var": tiny.two_var,
@@ -57,6 +75,9 @@ CASES = {
     "uc0": lambda: uc_config(0),
     "uc1": lambda: uc_config(1),
     "random_2e4": lambda: random_lp(20_000, 21),
+    "tuned_presolve": lambda: uc_config("tuned_presolve"),        # the shape PAPER.md l.232 / Table VI is about
+    "uc1_shuffled": lambda: shuffled_in_rows(uc_config(1), 7),
+    "ragged_shuffled": lambda: shuffled_in_rows(ragged_lp(), 8),
 }
 _lp_cache = {}
 
@@ -246,6 +267,61 @@ def test_trajectory_parity_200_attempts(name):
 
 def test_trajectory_parity_uc2_medium():
     assert_trajectory_parity(uc_config(2), 200)
+
+
+@pytest.mark.parametrize("name", ["uc1_shuffled", "ragged_shuffled"])
+def test_rows_stored_in_any_column_order_pass_the_layout_checks(name):
+    """Unsorted rows through the host self-check (entries kept in the caller's order) and the device-vs-host ingest
+    comparison; their 200-attempt parity runs with the other CASES."""
+    lp = get_lp(name)
+    from paper_2607_03627_b200.binding import host_layout_selftest
+    host_layout_selftest(lp)
+    host_layout_selftest(lp, sell_window=64, long_row_threshold=3)
+    with P.UcLp(lp, ruiz_iters=0, pc_alpha=0.0) as h:
+        h.compare_layout(lp)
+    with P.UcLp(lp, sell_window=64, long_row_threshold=3, ruiz_iters=0, pc_alpha=0.0) as h:
+        h.compare_layout(lp)
+
+
+@pytest.mark.parametrize("big", [1e20, 1e30])
+def test_finite_sentinel_bounds_are_absent_bounds_on_both_sides(big):
+    """R13: |bound| >= 1e20 means "no bound".  uc_config(0) with every infinite bound written as +-1e20
+    / +-1e30 must give, on each side, the very bits of the +-inf run -- and the GPU run the oracle's trajectory."""
+    import copy
+    lp = get_lp("uc0")
+    q = copy.copy(lp)
+    q.l = np.where(np.isneginf(lp.l), -big, lp.l); q.u = np.where(np.isposinf(lp.u), big, lp.u)
+    assert (np.isinf(lp.l).sum() + np.isinf(lp.u).sum()) > 0 and not np.isinf(q.l).any() and not np.isinf(q.u).any()
+    so_inf = oracle.solve(lp, fixed_iterations=200); so_big = oracle.solve(q, fixed_iterations=200)
+    np.testing.assert_array_equal(so_big.x, so_inf.x); np.testing.assert_array_equal(so_big.y, so_inf.y)
+    assert (so_big.primal_obj, so_big.dual_obj, so_big.rel_kkt) == (so_inf.primal_obj, so_inf.dual_obj, so_inf.rel_kkt)
+    with P.UcLp(lp) as a, P.UcLp(q) as b:
+        sa = a.solve(fixed_iterations=200, trace_attempts=200); sb = b.solve(fixed_iterations=200, trace_attempts=200)
+    np.testing.assert_array_equal(sb.x, sa.x); np.testing.assert_array_equal(sb.y, sa.y)
+    np.testing.assert_array_equal(sb.attempts["eta_used"], sa.attempts["eta_used"])
+    assert (sb.primal_obj, sb.dual_obj, sb.rel_kkt) == (sa.primal_obj, sa.dual_obj, sa.rel_kkt)
+    assert_trajectory_parity(q, 200)
+
+
+@pytest.mark.parametrize("what,k_fail", [("matrix", 1), ("cost", 64), ("rhs_tiny_matrix", 64)])
+def test_overflowing_input_ends_in_numerical_error_at_the_oracles_attempt(what, k_fail):
+    """R12: a non-finite step size stops the run at that attempt (the step rule in the dual kernel), a non-finite KKT term at
+    the next check.  Without preconditioning, entries of 1e200 overflow dx'K'dy in the first attempt; a cost of 1e308
+    or a right-hand side of 1e200 over a 1e-200 matrix overflow the objectives at the first check."""
+    import copy
+    q = copy.copy(get_lp("small_random"))
+    if what == "matrix":
+        q.val = q.val * 1e200
+    elif what == "cost":
+        q.c = q.c / np.abs(q.c).max() * 1e308
+    else:
+        q.val = q.val * 1e-200; q.b = q.b * 1e200
+    so = oracle.solve(q, ruiz_iters=0, pc_alpha=0.0, iter_limit=1000)
+    assert so.status == 4 and so.iterations == k_fail
+    with P.UcLp(q, ruiz_iters=0, pc_alpha=0.0) as h:
+        sg = h.solve(iter_limit=1000)
+        assert sg.status == P.NUMERICAL_ERROR and sg.iterations == so.iterations
+        assert h.solve(iter_limit=1000).status == P.NUMERICAL_ERROR       # and the handle survives it
 
 
 @pytest.mark.parametrize("window,thr", [(32, 4), (64, 1), (100000, 1000)])
