@@ -15,12 +15,16 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "pdhg_oracle.c")
-_LIB = os.path.join(_HERE, "libpdhg_oracle.so")
+# PDHG_ORACLE_LIB: load another build of the same source instead (the -fsanitize=address,undefined build of
+# profiles/r03_oracle_sanitizers.md); it is never built or rebuilt from here
+_LIB = os.environ.get("PDHG_ORACLE_LIB") or os.path.join(_HERE, "libpdhg_oracle.so")
 CFLAGS = ["-O2", "-ffp-contract=off", "-fno-fast-math", "-std=c11", "-shared", "-fPIC", "-Wall"]
 
 
 def build(force: bool = False) -> str:
     """Compile the oracle with gcc (single thread, no FMA contraction)."""
+    if os.environ.get("PDHG_ORACLE_LIB"):
+        return _LIB
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
         tmp = _LIB + f".tmp{os.getpid()}"
         subprocess.check_call(["gcc", *CFLAGS, _SRC, "-o", tmp, "-lm"])

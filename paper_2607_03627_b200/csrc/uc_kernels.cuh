@@ -19,6 +19,7 @@
 #include <stddef.h>
 #include <assert.h>
 #include "../../include/uc_pdhg.h"
+#include "../../include/uc_pdhg_hooks.h"
 #include "uc_dd.cuh"
 #include "uc_format.hpp"
 

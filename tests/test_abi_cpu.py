@@ -1,5 +1,5 @@
 """CPU-side checks of the boundary (no GPU): the C-ABI library loads and exports every symbol that
-include/uc_pdhg.h declares, struct layouts match the header, argument validation answers before any
+include/uc_pdhg.h and include/uc_pdhg_hooks.h declare, struct layouts match the header, argument validation answers before any
 device is touched, and the product path fails loudly (never falls back) without a GPU."""
 import ctypes as C
 import math
@@ -17,7 +17,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
 def header_functions():
-    src = open(os.path.join(ROOT, "include", "uc_pdhg.h")).read()
+    src = "".join(open(os.path.join(ROOT, "include", h)).read() for h in ("uc_pdhg.h", "uc_pdhg_hooks.h"))
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
     return sorted(set(re.findall(r"\b(uc_[a-z0-9_]+)\s*\(", src)))
 
@@ -29,6 +29,10 @@ def test_library_exports_every_declared_symbol():
     for n in names:
         assert hasattr(lib, n), n
     assert set(binding.EXPORTS) == set(names)
+    # the product header carries no measurement or test hook; they live in uc_pdhg_hooks.h
+    product = re.sub(r"/\*.*?\*/", "", open(os.path.join(ROOT, "include", "uc_pdhg.h")).read(), flags=re.S)
+    for hook in ("uc_pdhg_time_kernels", "uc_pdhg_timeline", "uc_lp_compare_layout", "uc_host_layout_selftest", "uc_host_log_rounded"):
+        assert hook not in product, hook
 
 
 def test_default_structs_match_header_values():
