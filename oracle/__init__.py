@@ -38,7 +38,7 @@ class Params(C.Structure):
                 ("fixed_iterations", C.c_int64), ("beta_sufficient", C.c_double),
                 ("beta_necessary", C.c_double), ("beta_artificial", C.c_double),
                 ("weight_smoothing", C.c_double), ("restarts_enabled", C.c_int32), ("pad_", C.c_int32),
-                ("frozen_eta", C.c_double)]
+                ("frozen_eta", C.c_double), ("eta0", C.c_double), ("omega0", C.c_double)]
 
 
 class Result(C.Structure):

@@ -51,6 +51,8 @@ typedef struct {
     int32_t restarts_enabled;  /* 1; 0 = checks still run, never restart (test hook) */
     int32_t pad_;
     double frozen_eta;         /* 0 = adaptive rule (R5); > 0: constant step, always accept (test hook) */
+    double eta0;               /* 0 = R2's 1/max|K~|; > 0: the step size the first attempt uses (R2b: state carried from an earlier solve) */
+    double omega0;             /* 0 = R2's ||c~||/||q~||; > 0: the primal weight the run starts with (R2b) */
 } oracle_params;
 
 typedef struct {
@@ -80,6 +82,7 @@ void oracle_default_params(oracle_params* p) {
     p->ruiz_iters = 10; p->pc_alpha = 1.0; p->fixed_iterations = 0;
     p->beta_sufficient = 0.2; p->beta_necessary = 0.8; p->beta_artificial = 0.36;
     p->weight_smoothing = 0.5; p->restarts_enabled = 1; p->pad_ = 0; p->frozen_eta = 0.0;
+    p->eta0 = 0.0; p->omega0 = 0.0;
 }
 
 /* ---------------------------------------------------------------- compensated sums */
@@ -310,6 +313,10 @@ int oracle_pdhg_solve(int64_t m, int64_t n, const int64_t* row_ptr, const int32_
     if (prm->frozen_eta > 0.0) eta = prm->frozen_eta;
     double ncs = sqrt(norm2sq(n, P.c)), nqs = sqrt(norm2sq(m, P.q));
     double omega = (ncs > 1e-10 && nqs > 1e-10) ? ncs / nqs : 1.0;
+    /* R2b: a re-solve may start from the step size and primal weight an
+       earlier solve of a neighbouring LP ended with, like it starts from its (x, y); everything else is R2..R14 unchanged */
+    if (prm->eta0 > 0.0 && prm->frozen_eta <= 0.0) eta = prm->eta0;
+    if (prm->omega0 > 0.0) omega = prm->omega0;
 
     int64_t k = 0, t0 = 0, accepted = 0, restarts = 0, na = 0, nc = 0;
     double w = 0.0, mu_prev = INFINITY;

@@ -504,6 +504,42 @@ def test_a_run_that_hits_its_iteration_limit_returns_the_better_of_current_and_a
     assert s.rel_kkt == pytest.approx(min(rc, ra) if s.check_w[-1] > 0.0 else rc, rel=1e-6)
 
 
+# ------------------------------------------------------------------ R2b: a run that starts from a supplied step size and primal weight
+def test_supplied_step_size_and_primal_weight_are_the_ones_the_first_attempt_and_check_use():
+    """R2b.  LP: min x s.t. x >= 1, x free; K = [1], c = q = 1, no preconditioning,
+    x0 = y0 = 0, a check after every attempt, eta0 = 0.5, omega0 = 4 (R2's own values would be 1 and 1).  By hand:
+      attempt 1: tau = eta/omega = 1/8, x' = 0 - (1 - 0)/8 = -1/8, xbar = -1/4; sigma = eta*omega = 2, y' = max(0, 0 + 2 (1 + 1/4)) = 5/2
+                 dx2 = 1/64, dy2 = 25/4, |dy K dx| = 5/16, eta_bar = (4/64 + 25/16) / (2 * 5/16) = 2.6 >= 0.5: accepted
+      check 1 (weight 4): current point: r_p = min(-1/8 - 1, 0) = -9/8, r_d = 1 - 5/2 = -3/2 (x free), gap = -1/8 - 5/2 = -21/8
+                 mu_c = sqrt(16 * 81/64 + (9/4)/16 + 441/64) = sqrt(27.28125)
+                 restart point (0, 0): r_p = -1, r_d = 1, gap = 0: mu_r = sqrt(16 + 1/16) = sqrt(16.0625)
+    Every value is exact in binary, so the comparisons are exact up to the square roots."""
+    from workloads.lp import from_dense
+    lp = from_dense([[1.0]], ["G"], [1.0], [1.0], [-np.inf], [np.inf], name="free_1x1")
+    kw = dict(ruiz_iters=0, pc_alpha=0.0, check_every=1, fixed_iterations=1, trace_attempts=1, trace_checks=1)
+    s = oracle.solve(lp, eta0=0.5, omega0=4.0, **kw)
+    a = s.attempts[0]
+    assert (a["eta_used"], a["dx2"], a["dy2"], a["inter"], a["eta_bar"], a["accepted"]) == (0.5, 1 / 64, 25 / 4, 5 / 16, 2.6, 1)
+    assert (s.x[0], s.y[0]) == (-0.125, 2.5)
+    kw2 = dict(kw, fixed_iterations=2, trace_attempts=2, trace_checks=2)         # the restart test runs only before the last attempt
+    c = oracle.solve(lp, eta0=0.5, omega0=4.0, **kw2).checks[0]
+    assert c["k"] == 1
+    assert c["mu_c"] == pytest.approx(np.sqrt(27.28125), rel=1e-15) and c["mu_r"] == pytest.approx(np.sqrt(16.0625), rel=1e-15)
+    # one at a time: the other one keeps R2's value (1 and 1 on this LP)
+    s = oracle.solve(lp, eta0=0.5, **kw)
+    assert (s.attempts[0]["eta_used"], s.x[0], s.y[0]) == (0.5, -0.5, 1.0)                  # tau = sigma = 1/2: x' = -1/2, y' = (1 + 1)/2
+    s = oracle.solve(lp, omega0=4.0, **kw)
+    assert (s.attempts[0]["eta_used"], s.x[0], s.y[0]) == (1.0, -0.25, 6.0)                 # tau = 1/4, sigma = 4: y' = 4 (1 + 1/2)
+    # 0 = not supplied: the run is R2's, bit for bit
+    d = oracle.solve(uc_config(0), fixed_iterations=130, trace_attempts=130)
+    z = oracle.solve(uc_config(0), fixed_iterations=130, trace_attempts=130, eta0=0.0, omega0=0.0)
+    np.testing.assert_array_equal(d.x, z.x); np.testing.assert_array_equal(d.attempts["eta_used"], z.attempts["eta_used"])
+    # and a run continued from the state of another ends where a longer run of the same attempts would not be reproduced
+    # exactly (k restarts from 1), but its first step size IS the supplied one
+    w = oracle.solve(uc_config(0), x0=d.x, y0=d.y, eta0=d.eta, omega0=d.omega, fixed_iterations=1, trace_attempts=1)
+    assert w.attempts["eta_used"][0] == d.eta
+
+
 # ------------------------------------------------------------------ library cross-check on the UC LP
 def test_uc_config0_converges_to_highs_objective():
     lp = uc_config(0)
