@@ -149,6 +149,9 @@ typedef struct {
     int64_t attempt_trace_cap;
     uc_check_record* check_trace;     /* nullable HOST buffer, check_trace_cap records */
     int64_t check_trace_cap;
+    double eta0;              /* 0 = R2's 1/max|K~|; > 0: step size of the first attempt (R2b) -- for re-solves: pass the eta and */
+    double omega0;            /* omega that uc_pdhg_result returned for the neighbouring LP, next to its (x, y) as x0 / y0.     */
+                              /* 0 = R2's ||c~||/||q~||; > 0: primal weight the run starts with (R2b).  Both must be finite, >= 0 */
 } uc_pdhg_params;
 
 void uc_pdhg_default_params(uc_pdhg_params* p);

@@ -32,7 +32,8 @@ class Params(C.Structure):
                 ("beta_artificial", C.c_double), ("weight_smoothing", C.c_double),
                 ("x0", C.c_void_p), ("y0", C.c_void_p), ("stream", C.c_void_p),
                 ("attempt_trace", C.c_void_p), ("attempt_trace_cap", C.c_int64),
-                ("check_trace", C.c_void_p), ("check_trace_cap", C.c_int64)]
+                ("check_trace", C.c_void_p), ("check_trace_cap", C.c_int64),
+                ("eta0", C.c_double), ("omega0", C.c_double)]
 
 
 class Result(C.Structure):

@@ -491,7 +491,9 @@ void start_run(uc_lp* lp, const uc_pdhg_params& prm, cudaStream_t st, long long 
                const double* dx0, const double* dy0, uc_attempt_record* d_att, uc_check_record* d_chk) {
     ensure_powtab(lp, std::min<long long>(limit, kPowtabStart));
     Ctrl h{};
-    h.eta = lp->eta0; h.omega = lp->omega0; h.eta_prev = 0.0; h.w = 0.0; h.mu_prev = INFINITY;
+    h.eta = prm.eta0 > 0.0 ? prm.eta0 : lp->eta0;                  // R2b: state carried over from an earlier solve, else R2
+    h.omega = prm.omega0 > 0.0 ? prm.omega0 : lp->omega0;
+    h.eta_prev = 0.0; h.w = 0.0; h.mu_prev = INFINITY;
     h.limit = limit; h.fixed = fixed ? 1 : 0; h.status = UC_ITERATION_LIMIT;
     h.eps_abs = prm.eps_abs; h.eps_rel = prm.eps_rel; h.beta_s = prm.beta_sufficient; h.beta_n = prm.beta_necessary;
     h.beta_a = prm.beta_artificial; h.smoothing = prm.weight_smoothing; h.norm_q = lp->norm_b; h.norm_c = lp->norm_c;
@@ -1097,7 +1099,8 @@ static int solve_impl(uc_lp* lp, const uc_pdhg_params* pin, double* x_out, doubl
     uc_pdhg_default_params(&prm);
     if (pin) prm = *pin;
     if (prm.check_every <= 0 || prm.iter_limit < 0 || prm.fixed_iterations < 0 || !(prm.eps_rel >= 0.0) || !(prm.eps_abs >= 0.0) ||
-        prm.attempt_trace_cap < 0 || prm.check_trace_cap < 0)
+        prm.attempt_trace_cap < 0 || prm.check_trace_cap < 0 || !(prm.eta0 >= 0.0) || !(prm.omega0 >= 0.0) ||
+        !std::isfinite(prm.eta0) || !std::isfinite(prm.omega0))
         return fail(UC_ERR_INVALID, "bad uc_pdhg_params");
     int expected = 0;
     if (!lp->busy.compare_exchange_strong(expected, 1)) return fail(UC_ERR_BUSY, "a solve is already running on this handle");

@@ -209,13 +209,15 @@ def cancel_latency(handle, after_s: float = 0.2, repeats: int = 5, **solve_kwarg
 
 
 def _main():
-    """python -m paper_2607_03627_b200.race --configs 0 1 2 [--poll 0.5] [--eps-abs 1e-4 1e-5] [--cancel-config 3]:
+    """python -m paper_2607_03627_b200.race --configs 0 1 2 tuned_presolve [--poll 0.5] [--eps-abs 1e-4 1e-5] [--cancel-config 3]:
     a Table-VI-style row per UC config and tolerance (which pipeline wins, P:l.221-226), with the CPU cores split evenly
     between the two pipelines (P:l.70), then the cancel latency of a solve in full flight."""
     import argparse
     from workloads import uc_config
     ap = argparse.ArgumentParser()
-    ap.add_argument("--configs", type=int, nargs="+", default=[0, 1])
+    ap.add_argument("--configs", type=lambda v: int(v) if v.lstrip("-").isdigit() else v, nargs="+", default=[0, 1],
+                    help="UC configs of BASELINE.json (0-3) or a named shape of workloads.uc_lp (tuned_presolve: the LP size the "
+                         "paper's tuned presolve leaves, P:l.232, the regime of Table VI)")
     ap.add_argument("--poll", type=float, default=0.5, help="poll period in s (0.5 in the paper, P:l.81)")
     ap.add_argument("--eps-abs", type=float, nargs="+", default=[1e-4], help="absolute tolerance(s); 1e-5 is the paper's knob (P:l.66)")
     ap.add_argument("--cancel-config", type=int, default=None)

@@ -18,6 +18,8 @@ def resolve_sequence(lp, fix_commitment, **solve_kwargs):
         relaxed                      the LP relaxation, cold
         dive_cold / dive_warm        a branch-and-bound style child: every commitment the relaxation left within 1e-3 of
                                      0 or 1 is fixed there (uc_lp_update_bounds); cold, and warm from the relaxed point
+        dive_state / cost_state      the same warm starts, carrying the parent's final step size and primal weight too
+                                     (uc_pdhg_params.eta0 / omega0, R2b)
         cost_cold / cost_warm        generation costs changed by +-2 % (uc_lp_update_objective), relaxed bounds; cold / warm
         fixed_cold / fixed_warm      the whole commitment fixed by rounding at 0.5 (may be infeasible: ramp and min-up/down
                                      rows do not survive rounding on every instance; PDHG then runs to its iteration limit)
@@ -44,12 +46,14 @@ def resolve_sequence(lp, fix_commitment, **solve_kwargs):
         h.update_bounds(l2.ravel(), u2.ravel())
         run(h, "dive_cold")
         run(h, "dive_warm", x0=r.x, y0=r.y)
+        run(h, "dive_state", x0=r.x, y0=r.y, eta0=r.eta, omega0=r.omega)
         h.update_bounds(lp.l, lp.u)
         # ---- cost change
         c2 = lp.c * (1.0 + 0.02 * np.sin(np.arange(lp.n) * 0.37))
         h.update_objective(c2)
         run(h, "cost_cold")
         run(h, "cost_warm", x0=r.x, y0=r.y)
+        run(h, "cost_state", x0=r.x, y0=r.y, eta0=r.eta, omega0=r.omega)
         h.update_objective(lp.c)
         # ---- the whole commitment rounded
         fixed = fix_commitment(lp, (U.T > 0.5).astype(float))
@@ -69,14 +73,14 @@ def _main():
     ap.add_argument("--configs", type=int, nargs="+", default=[0, 1, 2])
     ap.add_argument("--iter-limit", type=int, default=100000)
     args = ap.parse_args()
-    print("| config | relaxed, cold: attempts (s) | integral commitments fixed (share): cold / warm | costs +-2 %: cold / warm | "
+    print("| config | relaxed, cold: attempts (s) | integral commitments fixed (share): cold / warm (x, y) / warm (x, y, eta, omega) | costs +-2 %: cold / warm / warm + state | "
           "whole commitment rounded: cold / warm | relaxed again, warm from the rounded run | objective relaxed / dive / rounded |")
     print("|---|---|---|---|---|---|---|")
     for c in args.configs:
         lp = uc_config(c)
         o, s = resolve_sequence(lp, fix_commitment, iter_limit=args.iter_limit)
         cell = lambda k: f"{o[k].iterations} ({s[k]:.3f}){'' if o[k].status == _b.OPTIMAL else ' ' + _b.STATUS_NAMES[o[k].status]}"
-        print(f"| {c} | {cell('relaxed')} | ({o['dive_fixed_share']:.2f}) {cell('dive_cold')} / {cell('dive_warm')} | {cell('cost_cold')} / {cell('cost_warm')} | "
+        print(f"| {c} | {cell('relaxed')} | ({o['dive_fixed_share']:.2f}) {cell('dive_cold')} / {cell('dive_warm')} / {cell('dive_state')} | {cell('cost_cold')} / {cell('cost_warm')} / {cell('cost_state')} | "
               f"{cell('fixed_cold')} / {cell('fixed_warm')} | {cell('relaxed_warm')} | "
               f"{o['relaxed'].primal_obj:.6g} / {o['dive_warm'].primal_obj:.6g} / {o['fixed_warm'].primal_obj:.6g} |", flush=True)
 

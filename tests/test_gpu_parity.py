@@ -584,6 +584,41 @@ def test_warm_started_fixed_commitment_resolve_matches_oracle():
     assert warm.iterations <= cold.iterations
 
 
+@pytest.mark.parametrize("name", ["uc0", "uc1"])
+def test_resolve_that_carries_step_size_and_primal_weight_matches_oracle(name):
+    """DESIGN.md R2b: a branch-and-bound style child -- commitments the relaxation left integral are
+    fixed with uc_lp_update_bounds -- re-solved from the parent's (x, y) AND its final eta, omega.  The oracle is given the
+    same child LP, point and state: same trajectory for 200 attempts, same attempt count and restart trace at 1e-4."""
+    import copy
+    lp = get_lp(name)
+    G, T, V, oU = lp.meta["G"], lp.meta["T"], lp.meta["V"], lp.meta["offsets"]["u"]
+    with P.UcLp(lp) as h:
+        parent = h.solve()
+        assert parent.status == P.OPTIMAL and parent.eta > 0 and parent.omega > 0
+        U = parent.x.reshape(T, V)[:, oU:oU + G]
+        l2 = lp.l.copy().reshape(T, V); u2 = lp.u.copy().reshape(T, V)
+        l2[:, oU:oU + G][U >= 1.0 - 1e-3] = 1.0; u2[:, oU:oU + G][U <= 1e-3] = 0.0
+        child = copy.copy(lp); child.l = l2.ravel(); child.u = u2.ravel()
+        h.update_bounds(child.l, child.u)
+        kw = dict(x0=parent.x, y0=parent.y, eta0=parent.eta, omega0=parent.omega)
+        g200 = h.solve(fixed_iterations=200, trace_attempts=200, trace_checks=8, **kw)
+        gconv = h.solve(trace_checks=4096, **kw)
+        with pytest.raises(P.UcError):
+            h.solve(eta0=-1.0)
+        with pytest.raises(P.UcError):
+            h.solve(omega0=float("inf"))
+    o200 = oracle.solve(child, fixed_iterations=200, trace_attempts=200, trace_checks=8, **kw)
+    oconv = oracle.solve(child, **kw)
+    assert g200.attempts["eta_used"][0] == parent.eta == o200.attempts["eta_used"][0]
+    np.testing.assert_array_equal(g200.attempts["accepted"], o200.attempts["accepted"])
+    np.testing.assert_allclose(g200.attempts["eta_used"], o200.attempts["eta_used"], rtol=1e-9)
+    np.testing.assert_array_equal(g200.checks["restart_kind"], o200.checks["restart_kind"])
+    assert rel_l2(g200.x, o200.x) <= TOL_ITER and rel_l2(g200.y, o200.y) <= TOL_ITER
+    assert g200.omega == pytest.approx(o200.omega, rel=1e-9)
+    assert gconv.status == P.OPTIMAL == oconv.status and gconv.iterations == oconv.iterations and gconv.restarts == oconv.restarts
+    assert abs(gconv.primal_obj - oconv.primal_obj) <= TOL_OBJ * (1 + abs(oconv.primal_obj))
+
+
 def test_update_objective_equals_a_fresh_handle_and_the_oracle():
     """uc_lp_update_objective: the handle behaves like one created with the new c (the scalings do not depend on c)."""
     from workloads.lp import LP
